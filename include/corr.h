@@ -1,0 +1,128 @@
+/* corr.h -- C ABI of the B200-native X-engine (the O(N^2) hot path of arXiv 1503.06203).
+ *
+ * For each frequency channel f the library accumulates, over the T time samples of a call,
+ *
+ *      A_f[x][y] = sum_t X_t[x] * conj(X_t[y])          0 <= x <= y < N
+ *
+ * i.e. Eq. (1) of the paper, Corr(X,Y) = XY* = (XRe*YRe + XIm*YIm, XIm*YRe - XRe*YIm)
+ * (PAPER.md:41-44), accumulated over time, upper triangle only because A is
+ * Hermitian (Eq. 2), every channel independent.
+ *
+ * Input format (PAPER.md:76 and Fig. 2 at :82): time-major, then frequency, then the N input
+ * elements; ONE BYTE per complex sample, Re and Im each a 4-bit offset-encoded ("excess-8")
+ * integer: stored nibble = value + 8, value in [-8, 7].  The paper's text does not say which
+ * nibble is which; this library fixes Re = high nibble, Im = low nibble:
+ *      byte = ((Re + 8) << 4) | (Im + 8).
+ *
+ * Output format ("signed 32+32-bit complex correlation products"): int32 pairs
+ * (Re, Im), dense upper triangle in row-major order:
+ *      vis[f][b(x,y)][0..1],   b(x,y) = x*N - x*(x-1)/2 + (y - x),   B = N(N+1)/2 per channel.
+ * The paper's tile-blocked output addressing and its output lock are not
+ * reproduced; see DESIGN.md.
+ *
+ * All arithmetic is exact integer arithmetic.  One time sample adds at most 128 to |Re| and 120
+ * to |Im|, so an output buffer is overflow-free while the TOTAL number of samples accumulated
+ * into it (over all calls with accumulate_flag != 0) is <= 16 777 215 = floor((2^31-1)/128).
+ * Beyond that the result is two's-complement wraparound; the library cannot see across calls and
+ * does not check.
+ *
+ * Threading: a plan may be executed repeatedly on one stream.  Concurrent corr_execute calls on
+ * the SAME plan from different streams or threads are not supported (the plan owns device
+ * scratch).  Different plans are independent.  corr_last_error() is thread-local.
+ *
+ * There is no CPU fallback: every entry point that computes needs a CUDA device of compute
+ * capability 10.0 (sm_100a) and fails with CORR_ERR_CUDA / CORR_ERR_UNSUPPORTED otherwise.
+ */
+#ifndef CORR_B200_H
+#define CORR_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct corr_plan corr_plan; /* opaque; owned by the library */
+
+/* CUDA stream handle, passed as a plain pointer (cudaStream_t / CUstream); NULL = default stream. */
+typedef void *corr_stream_t;
+
+enum {
+    CORR_OK = 0,
+    CORR_ERR_INVALID_ARG = 1, /* bad N/F/T, NULL or misaligned pointer, NULL plan */
+    CORR_ERR_UNSUPPORTED = 2, /* device is not sm_100, or forced path cannot serve this shape */
+    CORR_ERR_ALLOC = 3,       /* host or device allocation failed */
+    CORR_ERR_CUDA = 4         /* a CUDA runtime/driver call or kernel launch failed */
+};
+
+/* Which kernel family a plan uses (S4 vs S4' of SURVEY.md S8(a)). */
+enum {
+    CORR_PATH_AUTO = 0,  /* library chooses from (N, F, T) */
+    CORR_PATH_DP4A = 1,  /* CUDA-core dp4a kernels; any N (small-N path) */
+    CORR_PATH_TCGEN05 = 2 /* TMA + tcgen05 int8 MMA, int32 accumulators in TMEM; needs N % 16 == 0 */
+};
+
+/* corr_plan_create -- validate the shape, choose the path, build the triangular tile schedule
+ * (only tiles on or above the diagonal) and allocate the plan's device scratch.
+ *   N  number of input elements,           N >= 1
+ *   F  number of frequency channels,       F >= 1
+ *   T  time samples per corr_execute call, 1 <= T <= 16 777 215
+ * Returns NULL on failure; the reason is in corr_last_error().  The environment variable
+ * CORR_FORCE_PATH=dp4a|tcgen05 overrides the automatic choice (testing aid). */
+corr_plan *corr_plan_create(int N, int F, int T);
+
+/* Same, with the path given explicitly (CORR_PATH_*).  CORR_ERR_UNSUPPORTED -> NULL if the
+ * path cannot serve the shape. */
+corr_plan *corr_plan_create_ex(int N, int F, int T, int path);
+
+/* corr_execute -- enqueue one correlation pass on `stream` and return without synchronising.
+ *   packed_dev  DEVICE pointer, T*F*N bytes, layout [T][F][N], format above; 16-byte aligned;
+ *               read only; must stay valid until the stream reaches the end of this call's work.
+ *   vis_dev     DEVICE pointer, F*N(N+1)/2*2 int32, layout [F][B][2] above; 8-byte aligned.
+ *   accumulate_flag  0: every entry of vis_dev is overwritten (whatever it held, including
+ *               Im = 0 on the diagonal); nonzero: the result is added, modulo 2^32, to what
+ *               vis_dev holds (the paper's output buffer persists across launches and is added
+ *               to).
+ *   stream      CUDA stream the work is enqueued on.
+ * Returns CORR_OK or an error code; errors found at enqueue time are returned here, later
+ * device faults surface at the caller's own synchronisation.  The caller owns both buffers. */
+int corr_execute(corr_plan *plan, const uint8_t *packed_dev, int32_t *vis_dev,
+                 int accumulate_flag, corr_stream_t stream);
+
+/* corr_execute_host -- the same pass with HOST buffers: copies packed_host to a plan-owned
+ * device buffer, runs corr_execute, copies the result back, all on `stream`, then synchronises
+ * the stream.  With accumulate_flag != 0 vis_host is first copied to the device and added to.
+ * Pinned host memory makes the copies asynchronous; pageable memory works but is slower. */
+int corr_execute_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_host,
+                      int accumulate_flag, corr_stream_t stream);
+
+/* corr_plan_destroy -- free the plan and its device scratch.  NULL is a no-op. */
+void corr_plan_destroy(corr_plan *plan);
+
+/* Thread-local, NUL-terminated description of the last failure in this thread; never NULL;
+ * owned by the library. */
+const char *corr_last_error(void);
+
+/* Pure host conveniences. */
+size_t corr_input_bytes(const corr_plan *plan);        /* T*F*N */
+size_t corr_vis_elems(const corr_plan *plan);          /* F * N(N+1)/2 * 2 int32 values */
+size_t corr_baseline_index(int N, int x, int y);       /* b(x,y); requires 0 <= x <= y < N, else (size_t)-1 */
+
+/* Plan introspection (host only).  Writes up to 8 ints:
+ *   info[0] path actually chosen (CORR_PATH_DP4A / CORR_PATH_TCGEN05)
+ *   info[1] tile edge in elements along x     info[2] tile edge along y
+ *   info[3] tiles per channel on or above the diagonal
+ *   info[4] T-slices per tile (split-T factor) info[5] total work units = F*tiles*slices
+ *   info[6] CTAs launched by the main kernel  info[7] kernels launched per corr_execute
+ * Returns CORR_OK or CORR_ERR_INVALID_ARG. */
+int corr_plan_info(const corr_plan *plan, int info[8]);
+
+/* Number of tiles of edge (tile_x, tile_y) that touch the upper triangle of an N x N matrix
+ * (host only; the scheduler's counting rule, Fig. 1: N=256, 32x32 -> 36). */
+int corr_count_tiles(int N, int tile_x, int tile_y);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CORR_B200_H */

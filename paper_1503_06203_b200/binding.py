@@ -1,0 +1,172 @@
+"""ctypes binding of include/corr.h.  Same names as the C ABI; argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+_LIB_PATH = _HERE / "libcorr_b200.so"
+
+PATH_AUTO, PATH_DP4A, PATH_TCGEN05 = 0, 1, 2
+
+# every symbol include/corr.h declares (tests check the library exports all of them)
+SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
+           "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles")
+
+
+class CorrError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib_path() -> Path:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libcorr_b200.so.  Fails loudly if it has not been built (python -m
+    paper_1503_06203_b200.build or __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise CorrError(f"{_LIB_PATH} not built; run __graft_entry__.build() - there is no fallback path")
+        lib = ctypes.CDLL(str(_LIB_PATH))
+        vp, ci, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+        lib.corr_plan_create.argtypes = [ci, ci, ci]
+        lib.corr_plan_create.restype = vp
+        lib.corr_plan_create_ex.argtypes = [ci, ci, ci, ci]
+        lib.corr_plan_create_ex.restype = vp
+        lib.corr_execute.argtypes = [vp, vp, vp, ci, vp]
+        lib.corr_execute.restype = ci
+        lib.corr_execute_host.argtypes = [vp, vp, vp, ci, vp]
+        lib.corr_execute_host.restype = ci
+        lib.corr_plan_destroy.argtypes = [vp]
+        lib.corr_plan_destroy.restype = None
+        lib.corr_last_error.argtypes = []
+        lib.corr_last_error.restype = ctypes.c_char_p
+        lib.corr_input_bytes.argtypes = [vp]
+        lib.corr_input_bytes.restype = sz
+        lib.corr_vis_elems.argtypes = [vp]
+        lib.corr_vis_elems.restype = sz
+        lib.corr_baseline_index.argtypes = [ci, ci, ci]
+        lib.corr_baseline_index.restype = sz
+        lib.corr_plan_info.argtypes = [vp, ctypes.POINTER(ci * 8)]
+        lib.corr_plan_info.restype = ci
+        lib.corr_count_tiles.argtypes = [ci, ci, ci]
+        lib.corr_count_tiles.restype = ci
+        _lib = lib
+    return _lib
+
+
+def _err() -> str:
+    return load_library().corr_last_error().decode(errors="replace")
+
+
+# ------------------------------------------------------------------ C-ABI names, 1:1
+def corr_plan_create(N: int, F: int, T: int, path: int = PATH_AUTO) -> int:
+    lib = load_library()
+    h = lib.corr_plan_create(N, F, T) if path == PATH_AUTO else lib.corr_plan_create_ex(N, F, T, path)
+    if not h:
+        raise CorrError(_err())
+    return h
+
+
+def corr_execute(plan: int, packed_dev_ptr: int, vis_dev_ptr: int, accumulate_flag: int, stream: int) -> None:
+    rc = load_library().corr_execute(plan, packed_dev_ptr, vis_dev_ptr, int(bool(accumulate_flag)), stream)
+    if rc != 0:
+        raise CorrError(f"corr_execute -> {rc}: {_err()}")
+
+
+def corr_execute_host(plan: int, packed_host_ptr: int, vis_host_ptr: int, accumulate_flag: int, stream: int) -> None:
+    rc = load_library().corr_execute_host(plan, packed_host_ptr, vis_host_ptr, int(bool(accumulate_flag)), stream)
+    if rc != 0:
+        raise CorrError(f"corr_execute_host -> {rc}: {_err()}")
+
+
+def corr_plan_destroy(plan: int) -> None:
+    load_library().corr_plan_destroy(plan)
+
+
+def baseline_index(N: int, x: int, y: int) -> int:
+    v = load_library().corr_baseline_index(N, x, y)
+    if v == ctypes.c_size_t(-1).value:
+        raise ValueError("need 0 <= x <= y < N")
+    return int(v)
+
+
+def count_tiles(N: int, tile_x: int, tile_y: int) -> int:
+    return int(load_library().corr_count_tiles(N, tile_x, tile_y))
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class Plan:
+    """corr_plan with torch tensors as device buffers (torch: allocation + streams only)."""
+
+    def __init__(self, N: int, F: int, T: int, path: int = PATH_AUTO):
+        self.N, self.F, self.T = N, F, T
+        self._h = corr_plan_create(N, F, T, path)
+        lib = load_library()
+        self.input_bytes = int(lib.corr_input_bytes(self._h))
+        self.vis_elems = int(lib.corr_vis_elems(self._h))
+        arr = (ctypes.c_int * 8)()
+        if lib.corr_plan_info(self._h, ctypes.byref(arr)) != 0:
+            raise CorrError(_err())
+        keys = ("path", "tile_x", "tile_y", "tiles_per_channel", "slices", "units", "ctas", "kernels")
+        self.info = dict(zip(keys, list(arr)))
+
+    @property
+    def baselines(self) -> int:
+        return self.N * (self.N + 1) // 2
+
+    def new_vis(self, device="cuda"):
+        import torch
+        return torch.empty((self.F, self.baselines, 2), dtype=torch.int32, device=device)
+
+    def execute(self, packed, vis=None, accumulate: bool = False, stream=None):
+        """packed: uint8 CUDA tensor [T][F][N]; vis: int32 CUDA tensor [F][B][2] (allocated if None).
+        Enqueues on `stream` (default: torch's current stream); does not synchronise."""
+        import torch
+        if not packed.is_cuda or packed.dtype != torch.uint8 or not packed.is_contiguous():
+            raise ValueError("packed must be a contiguous uint8 CUDA tensor")
+        if packed.numel() != self.input_bytes:
+            raise ValueError(f"packed has {packed.numel()} bytes, plan expects {self.input_bytes}")
+        if vis is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs an existing vis tensor")
+            vis = self.new_vis(packed.device)
+        if not vis.is_cuda or vis.dtype != torch.int32 or not vis.is_contiguous() or vis.numel() != self.vis_elems:
+            raise ValueError("vis must be a contiguous int32 CUDA tensor of F*B*2 elements")
+        s = torch.cuda.current_stream(packed.device) if stream is None else stream
+        corr_execute(self._h, packed.data_ptr(), vis.data_ptr(), int(accumulate), s.cuda_stream)
+        return vis
+
+    def execute_host(self, packed_host, vis_host, accumulate: bool = False, stream=None):
+        """packed_host / vis_host: CPU torch tensors (pinned for async copies) or numpy arrays."""
+        import torch
+        s = torch.cuda.current_stream() if stream is None else stream
+
+        def ptr(a):
+            return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+
+        corr_execute_host(self._h, ptr(packed_host), ptr(vis_host), int(accumulate), s.cuda_stream)
+        return vis_host
+
+    def close(self):
+        if getattr(self, "_h", None):
+            corr_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,355 @@
+// corr_api.cu -- the C ABI of include/corr.h: plan construction (path choice, triangular tile
+// schedule = step S3), TMA tensor-map construction, kernel launches.  Host code only; the
+// kernels are in corr_dp4a.cuh (S4') and corr_tc.cuh (S1, S2, S4, S5).
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "../../include/corr.h"
+#include "corr_dp4a.cuh"
+#include "corr_tc.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+void set_err(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+#define CUDA_TRY(expr, code)                                                          \
+    do {                                                                              \
+        cudaError_t e_ = (expr);                                                      \
+        if (e_ != cudaSuccess) {                                                      \
+            set_err("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return code;                                                              \
+        }                                                                             \
+    } while (0)
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                   CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+int count_tiles(int N, int tx, int ty)
+{
+    // tile (bx, by) covers x in [bx*tx, (bx+1)*tx), y in [by*ty, (by+1)*ty); it touches the upper
+    // triangle iff its largest y is >= its smallest x.
+    if (N < 1 || tx < 1 || ty < 1) return -1;
+    const int nbx = (N + tx - 1) / tx, nby = (N + ty - 1) / ty;
+    int n = 0;
+    for (int bx = 0; bx < nbx; ++bx)
+        for (int by = 0; by < nby; ++by)
+            if (std::min(N, (by + 1) * ty) - 1 >= bx * tx) ++n;
+    return n;
+}
+
+}  // namespace
+
+struct corr_plan {
+    int N, F, T, path;
+    int sm_count;
+    // schedule
+    int tile;          // tile edge (square tiles)
+    int tiles_per_f;
+    int slices;        // T-slices per tile
+    int t_per_slice;
+    int num_units;
+    int grid;
+    int kernels_per_exec;
+    ushort2 *tiles_dev;
+    // dp4a only
+    int aligned;
+    // tcgen05 only
+    CUtensorMap tmap;
+    const void *tmap_ptr;
+    // corr_execute_host staging
+    uint8_t *packed_own;
+    int32_t *vis_own;
+};
+
+extern "C" {
+
+const char *corr_last_error(void) { return g_err; }
+
+size_t corr_baseline_index(int N, int x, int y)
+{
+    if (N < 1 || x < 0 || y < x || y >= N) return (size_t)-1;
+    return (size_t)x * N - (size_t)x * (x - 1) / 2 + (size_t)(y - x);
+}
+
+int corr_count_tiles(int N, int tile_x, int tile_y) { return count_tiles(N, tile_x, tile_y); }
+
+size_t corr_input_bytes(const corr_plan *p) { return p ? (size_t)p->T * p->F * p->N : 0; }
+
+size_t corr_vis_elems(const corr_plan *p) { return p ? (size_t)p->F * ((size_t)p->N * (p->N + 1) / 2) * 2 : 0; }
+
+int corr_plan_info(const corr_plan *p, int info[8])
+{
+    if (!p || !info) {
+        set_err("corr_plan_info: NULL argument");
+        return CORR_ERR_INVALID_ARG;
+    }
+    info[0] = p->path;
+    info[1] = p->tile;
+    info[2] = p->tile;
+    info[3] = p->tiles_per_f;
+    info[4] = p->slices;
+    info[5] = p->num_units;
+    info[6] = p->grid;
+    info[7] = p->kernels_per_exec;
+    return CORR_OK;
+}
+
+void corr_plan_destroy(corr_plan *p)
+{
+    if (!p) return;
+    if (p->tiles_dev) cudaFree(p->tiles_dev);
+    if (p->packed_own) cudaFree(p->packed_own);
+    if (p->vis_own) cudaFree(p->vis_own);
+    delete p;
+}
+
+corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
+{
+    if (N < 1 || F < 1 || T < 1 || T > 16777215) {
+        set_err("corr_plan_create: need N >= 1, F >= 1, 1 <= T <= 16777215 (got N=%d F=%d T=%d)", N, F, T);
+        return nullptr;
+    }
+    if (N > 65535 * 16) {
+        set_err("corr_plan_create: N=%d too large for the tile table", N);
+        return nullptr;
+    }
+    if (path != CORR_PATH_AUTO && path != CORR_PATH_DP4A && path != CORR_PATH_TCGEN05) {
+        set_err("corr_plan_create: unknown path %d", path);
+        return nullptr;
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        set_err("corr_plan_create: no usable CUDA device (%s); this library has no CPU fallback",
+                cudaGetErrorString(cudaGetLastError()));
+        return nullptr;
+    }
+    if (prop.major != 10) {
+        set_err("corr_plan_create: device '%s' is sm_%d%d; this library is built for sm_100a only", prop.name,
+                prop.major, prop.minor);
+        return nullptr;
+    }
+    if (path == CORR_PATH_AUTO) {
+        const char *force = getenv("CORR_FORCE_PATH");
+        if (force && !strcmp(force, "dp4a"))
+            path = CORR_PATH_DP4A;
+        else if (force && !strcmp(force, "tcgen05"))
+            path = CORR_PATH_TCGEN05;
+        else
+            path = (N % 16 == 0 && N >= 96) ? CORR_PATH_TCGEN05 : CORR_PATH_DP4A;
+    }
+    if (path == CORR_PATH_TCGEN05 && N % 16 != 0) {
+        set_err("corr_plan_create: the tcgen05 path needs N %% 16 == 0 (TMA row stride), got N=%d", N);
+        return nullptr;
+    }
+
+    corr_plan *p = new (std::nothrow) corr_plan();
+    if (!p) {
+        set_err("corr_plan_create: out of host memory");
+        return nullptr;
+    }
+    memset(p, 0, sizeof(*p));
+    p->N = N;
+    p->F = F;
+    p->T = T;
+    p->path = path;
+    p->sm_count = prop.multiProcessorCount;
+
+    // ---- S3: the triangular tile table (only tiles on or above the diagonal)
+    if (path == CORR_PATH_DP4A)
+        p->tile = (N <= 16) ? 16 : (N <= 32) ? 32 : 64;
+    else
+        p->tile = corr::TC_BLK;
+    const int nb = (N + p->tile - 1) / p->tile;
+    std::vector<ushort2> tiles;
+    for (int bx = 0; bx < nb; ++bx)
+        for (int by = bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
+    p->tiles_per_f = (int)tiles.size();
+    const long long units0 = (long long)F * p->tiles_per_f;
+    if (units0 > 0x7fffffffLL / 64) {
+        set_err("corr_plan_create: too many work units");
+        delete p;
+        return nullptr;
+    }
+
+    // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
+    const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK : corr::TC_ST;
+    const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : corr::TC_MAX_SLICE;
+    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : p->sm_count;
+    const double per_sample = (path == CORR_PATH_DP4A) ? 40.0 : 8.0;  // cycles per time sample per unit
+    const double epi = (path == CORR_PATH_DP4A) ? 1500.0 : 6000.0;    // cycles per unit, fixed
+    const int min_slices = (T + max_slice - 1) / max_slice;
+    double best_cost = 0;
+    int best_s = 0;
+    for (int s = min_slices; s <= std::max(min_slices, 64); ++s) {
+        int tps = ((T + s - 1) / s + quantum - 1) / quantum * quantum;
+        if (s > min_slices && tps < 8 * quantum) break;
+        const int s_eff = (T + tps - 1) / tps;
+        const double waves = (double)((units0 * s_eff + ctas_per_wave - 1) / ctas_per_wave);
+        const double cost = waves * (per_sample * tps + epi * (s_eff > 1 ? 2.0 : 1.0));
+        if (best_s == 0 || cost < best_cost * 0.97) {
+            best_cost = cost;
+            best_s = s;
+        }
+    }
+    p->t_per_slice = ((T + best_s - 1) / best_s + quantum - 1) / quantum * quantum;
+    p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
+    p->num_units = (int)(units0 * p->slices);
+    p->grid = (path == CORR_PATH_DP4A) ? p->num_units : std::min(p->num_units, p->sm_count);
+    p->kernels_per_exec = 1;
+    p->aligned = (N % 4 == 0) ? 1 : 0;
+
+    if (cudaMalloc(&p->tiles_dev, tiles.size() * sizeof(ushort2)) != cudaSuccess ||
+        cudaMemcpy(p->tiles_dev, tiles.data(), tiles.size() * sizeof(ushort2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        set_err("corr_plan_create: device allocation of the tile table failed: %s",
+                cudaGetErrorString(cudaGetLastError()));
+        corr_plan_destroy(p);
+        return nullptr;
+    }
+    if (path == CORR_PATH_TCGEN05) {
+        if (!get_encode_fn()) {
+            set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
+            corr_plan_destroy(p);
+            return nullptr;
+        }
+        if (cudaFuncSetAttribute(corr::corr_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 corr::TC_SMEM_BYTES) != cudaSuccess) {
+            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::TC_SMEM_BYTES,
+                    cudaGetErrorString(cudaGetLastError()));
+            corr_plan_destroy(p);
+            return nullptr;
+        }
+    }
+    return p;
+}
+
+corr_plan *corr_plan_create(int N, int F, int T) { return corr_plan_create_ex(N, F, T, CORR_PATH_AUTO); }
+
+static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
+{
+    if (p->tmap_ptr == packed_dev) return CORR_OK;
+    // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
+    const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
+    const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
+    const cuuint32_t box[3] = {(cuuint32_t)corr::TC_BLK, 1u, (cuuint32_t)corr::TC_ST};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
+                                 strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_err("cuTensorMapEncodeTiled failed with CUresult %d (N=%d F=%d T=%d)", (int)r, p->N, p->F, p->T);
+        return CORR_ERR_CUDA;
+    }
+    p->tmap_ptr = packed_dev;
+    return CORR_OK;
+}
+
+int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int accumulate_flag,
+                 corr_stream_t stream_)
+{
+    if (!p || !packed_dev || !vis_dev) {
+        set_err("corr_execute: NULL plan or buffer");
+        return CORR_ERR_INVALID_ARG;
+    }
+    if ((reinterpret_cast<uintptr_t>(packed_dev) & 15u) || (reinterpret_cast<uintptr_t>(vis_dev) & 7u)) {
+        set_err("corr_execute: packed_dev must be 16-byte aligned and vis_dev 8-byte aligned");
+        return CORR_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    int out_mode;
+    if (p->slices > 1) {
+        out_mode = corr::OUT_ATOMIC;
+        if (!accumulate_flag)
+            CUDA_TRY(cudaMemsetAsync(vis_dev, 0, corr_vis_elems(p) * sizeof(int32_t), stream), CORR_ERR_CUDA);
+    } else {
+        out_mode = accumulate_flag ? corr::OUT_RMW : corr::OUT_STORE;
+    }
+
+    if (p->path == CORR_PATH_DP4A) {
+        dim3 grid((unsigned)(p->F * p->tiles_per_f), (unsigned)p->slices);
+        switch (p->tile) {
+        case 16:
+            corr::corr_dp4a_kernel<16><<<grid, corr::DP4A_THREADS, 0, stream>>>(
+                packed_dev, vis_dev, p->tiles_dev, p->tiles_per_f, p->N, p->F, p->T, p->t_per_slice, out_mode, p->aligned);
+            break;
+        case 32:
+            corr::corr_dp4a_kernel<32><<<grid, corr::DP4A_THREADS, 0, stream>>>(
+                packed_dev, vis_dev, p->tiles_dev, p->tiles_per_f, p->N, p->F, p->T, p->t_per_slice, out_mode, p->aligned);
+            break;
+        default:
+            corr::corr_dp4a_kernel<64><<<grid, corr::DP4A_THREADS, 0, stream>>>(
+                packed_dev, vis_dev, p->tiles_dev, p->tiles_per_f, p->N, p->F, p->T, p->t_per_slice, out_mode, p->aligned);
+            break;
+        }
+    } else {
+        int rc = build_tmap(p, packed_dev);
+        if (rc != CORR_OK) return rc;
+        corr::TcParams prm;
+        prm.N = p->N;
+        prm.F = p->F;
+        prm.T = p->T;
+        prm.tiles_per_f = p->tiles_per_f;
+        prm.slices = p->slices;
+        prm.t_per_slice = p->t_per_slice;
+        prm.num_units = p->num_units;
+        prm.out_mode = out_mode;
+        prm.tiles = p->tiles_dev;
+        prm.vis = vis_dev;
+        corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
+    }
+    CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+    return CORR_OK;
+}
+
+int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_host, int accumulate_flag,
+                      corr_stream_t stream_)
+{
+    if (!p || !packed_host || !vis_host) {
+        set_err("corr_execute_host: NULL plan or buffer");
+        return CORR_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t in_bytes = corr_input_bytes(p), out_bytes = corr_vis_elems(p) * sizeof(int32_t);
+    if (!p->packed_own) CUDA_TRY(cudaMalloc(&p->packed_own, in_bytes), CORR_ERR_ALLOC);
+    if (!p->vis_own) CUDA_TRY(cudaMalloc(&p->vis_own, out_bytes), CORR_ERR_ALLOC);
+    CUDA_TRY(cudaMemcpyAsync(p->packed_own, packed_host, in_bytes, cudaMemcpyHostToDevice, stream), CORR_ERR_CUDA);
+    if (accumulate_flag)
+        CUDA_TRY(cudaMemcpyAsync(p->vis_own, vis_host, out_bytes, cudaMemcpyHostToDevice, stream), CORR_ERR_CUDA);
+    int rc = corr_execute(p, p->packed_own, p->vis_own, accumulate_flag, stream_);
+    if (rc != CORR_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(vis_host, p->vis_own, out_bytes, cudaMemcpyDeviceToHost, stream), CORR_ERR_CUDA);
+    CUDA_TRY(cudaStreamSynchronize(stream), CORR_ERR_CUDA);
+    return CORR_OK;
+}
+
+}  // extern "C"
