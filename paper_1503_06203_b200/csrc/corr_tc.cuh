@@ -28,11 +28,11 @@
 // the unpack is a 16-byte load, 3 logic ops per word and two 16-byte stores at the same offset,
 // with no transpose and no bank conflicts.
 //
-// Warp roles (320 threads, 1 CTA per SM, persistent over work units):
-//   warp 0      TMA producer (packed bytes -> pk ring)
-//   warp 1      TMEM owner + MMA issuer (one elected thread)
-//   warps 2-5   unpack (pk ring -> operand-plane ring)
-//   warps 6-9   epilogue (TMEM -> registers -> smem transpose -> vis)
+// Warp roles (448 threads, 1 CTA per SM, persistent over work units):
+//   warp 0       TMA producer (packed bytes -> pk ring)
+//   warp 1       TMEM owner + MMA issuer (one elected thread)
+//   warps 2-9    unpack (pk ring -> operand-plane ring)
+//   warps 10-13  epilogue (TMEM -> registers -> smem transpose -> vis)
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -45,9 +45,12 @@ namespace corr {
 
 constexpr int TC_BLK = 128;            // tile edge (inputs)
 constexpr int TC_ST = 64;              // time samples per pipeline stage
-constexpr int TC_PK_STAGES = 3;        // packed-byte ring depth
+constexpr int TC_PK_STAGES = 6;        // packed-byte ring depth (covers TMA latency)
 constexpr int TC_PL_STAGES = 3;        // operand-plane ring depth
-constexpr int TC_THREADS = 320;
+constexpr int TC_UNPACK_WARPS = 8;
+constexpr int TC_UNPACK_THREADS = 32 * TC_UNPACK_WARPS;
+constexpr int TC_EPI_WARP0 = 2 + TC_UNPACK_WARPS;  // first epilogue warp
+constexpr int TC_THREADS = 32 * (TC_EPI_WARP0 + 4);
 constexpr int TC_PLANE = TC_ST * TC_BLK;            // bytes of one operand plane per stage
 constexpr int TC_PK_BYTES = 2 * TC_PLANE;           // X and Y packed blocks
 constexpr int TC_PL_BYTES = 4 * TC_PLANE;           // Ar, Ai, Br, Bi
@@ -96,10 +99,10 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         ptx::prefetch_tmap(&tmap);
         for (int s = 0; s < TC_PK_STAGES; ++s) {
             ptx::mbar_init(pk_full(s), 1);
-            ptx::mbar_init(pk_empty(s), 4);
+            ptx::mbar_init(pk_empty(s), TC_UNPACK_WARPS);
         }
         for (int s = 0; s < TC_PL_STAGES; ++s) {
-            ptx::mbar_init(pl_full(s), 4);
+            ptx::mbar_init(pl_full(s), TC_UNPACK_WARPS);
             ptx::mbar_init(pl_empty(s), 1);
         }
         ptx::mbar_init(acc_full, 1);
@@ -186,9 +189,9 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 acc_ph ^= 1u;
             }
         }
-    } else if (warp < 6) {
+    } else if (warp < TC_EPI_WARP0) {
         // ===================== S2: unpack =====================
-        const int ut = threadIdx.x - 64;  // 0..127
+        const int ut = threadIdx.x - 64;  // 0..TC_UNPACK_THREADS-1
         int pst = 0, qst = 0;
         uint32_t pph = 0, qph = 0;
         for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
@@ -205,23 +208,30 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 const uint32_t src = pk0 + pst * TC_PK_BYTES;
                 const uint32_t dst = pl0 + qst * TC_PL_BYTES;
                 const int nblk = diag ? 1 : 2;
+                constexpr int CH = TC_PLANE / 16 / TC_UNPACK_THREADS;  // 16-byte chunks per thread per block
+                const uint8_t *srcg = gbase + (src - base);
+                uint8_t *dstg = gbase + (dst - base);
+                uint4 w[2][CH];
+                // all loads of the stage first (independent, several in flight), then logic + stores
+                for (int b = 0; b < nblk; ++b)
+#pragma unroll
+                    for (int k = 0; k < CH; ++k)
+                        w[b][k] = *reinterpret_cast<const uint4 *>(srcg + b * TC_PLANE +
+                                                                   (k * TC_UNPACK_THREADS + ut) * 16);
                 for (int b = 0; b < nblk; ++b) {
 #pragma unroll
-                    for (int k = 0; k < TC_PLANE / 16 / 128; ++k) {
-                        const uint32_t off = (uint32_t)(k * 128 + ut) * 16u;
-                        uint32_t w0, w1, w2, w3;
-                        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
-                                     : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3)
-                                     : "r"(src + b * TC_PLANE + off));
+                    for (int k = 0; k < CH; ++k) {
+                        const uint32_t off = (uint32_t)(k * TC_UNPACK_THREADS + ut) * 16u;
                         const bool ok = (int)(off >> 7) < rows_valid;
                         const uint32_t m = ok ? 0xF0F0F0F0u : 0u;
-                        const uint32_t r0 = (w0 ^ 0x80808080u) & m, r1 = (w1 ^ 0x80808080u) & m;
-                        const uint32_t r2 = (w2 ^ 0x80808080u) & m, r3 = (w3 ^ 0x80808080u) & m;
-                        const uint32_t i0 = ((w0 << 4) ^ 0x80808080u) & m, i1 = ((w1 << 4) ^ 0x80808080u) & m;
-                        const uint32_t i2 = ((w2 << 4) ^ 0x80808080u) & m, i3 = ((w3 << 4) ^ 0x80808080u) & m;
-                        const uint32_t o = dst + b * 2 * TC_PLANE + off;
-                        asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(o), "r"(r0), "r"(r1), "r"(r2), "r"(r3) : "memory");
-                        asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(o + TC_PLANE), "r"(i0), "r"(i1), "r"(i2), "r"(i3) : "memory");
+                        const uint4 v = w[b][k];
+                        uint4 r, i;
+                        r.x = (v.x ^ 0x80808080u) & m; r.y = (v.y ^ 0x80808080u) & m;
+                        r.z = (v.z ^ 0x80808080u) & m; r.w = (v.w ^ 0x80808080u) & m;
+                        i.x = ((v.x << 4) ^ 0x80808080u) & m; i.y = ((v.y << 4) ^ 0x80808080u) & m;
+                        i.z = ((v.z << 4) ^ 0x80808080u) & m; i.w = ((v.w << 4) ^ 0x80808080u) & m;
+                        *reinterpret_cast<uint4 *>(dstg + b * 2 * TC_PLANE + off) = r;
+                        *reinterpret_cast<uint4 *>(dstg + b * 2 * TC_PLANE + TC_PLANE + off) = i;
                     }
                 }
                 ptx::fence_proxy_async_smem();  // planes were written by the generic proxy; MMA reads via async proxy
@@ -237,7 +247,7 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     } else {
         // ===================== S5: epilogue =====================
         const int q = warp & 3;  // TMEM lane quarter this warp may read
-        uint8_t *stage = epi_g + (warp - 6) * 32 * TC_EPI_PITCH;
+        uint8_t *stage = epi_g + (warp - TC_EPI_WARP0) * 32 * TC_EPI_PITCH;
         const size_t Bn = (size_t)p.N * ((size_t)p.N + 1) / 2;
         uint32_t acc_ph = 0;
         for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
