@@ -14,6 +14,7 @@
 #include "../../include/corr.h"
 #include "corr_dp4a.cuh"
 #include "corr_tc.cuh"
+#include "corr_tc2.cuh"
 
 namespace {
 
@@ -84,7 +85,9 @@ struct corr_plan {
     // dp4a only
     int aligned;
     // tcgen05 only
+    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128 (corr_tc2.cuh)
     CUtensorMap tmap;
+    CUtensorMap tmap_y;
     const void *tmap_ptr;
     // corr_execute_host staging
     uint8_t *packed_own;
@@ -114,7 +117,7 @@ int corr_plan_info(const corr_plan *p, int info[8])
         return CORR_ERR_INVALID_ARG;
     }
     info[0] = p->path;
-    info[1] = p->tile;
+    info[1] = (p->variant == 2) ? 256 : p->tile;
     info[2] = p->tile;
     info[3] = p->tiles_per_f;
     info[4] = p->slices;
@@ -190,10 +193,23 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->tile = (N <= 16) ? 16 : (N <= 32) ? 32 : 64;
     else
         p->tile = corr::TC_BLK;
+    p->variant = 0;
+    if (path == CORR_PATH_TCGEN05) {
+        const char *v = getenv("CORR_TC_VARIANT");
+        p->variant = (v && !strcmp(v, "1")) ? 1 : 2;
+    }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
-    for (int bx = 0; bx < nb; ++bx)
-        for (int by = bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
+    if (p->variant == 2) {
+        // pair tiles: x-block of 256 (two CTAs x 128), y-block of 128; keep those whose largest y
+        // reaches their smallest x
+        const int nbx = (N + 255) / 256;
+        for (int bx = 0; bx < nbx; ++bx)
+            for (int by = 2 * bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
+    } else {
+        for (int bx = 0; bx < nb; ++bx)
+            for (int by = bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
+    }
     p->tiles_per_f = (int)tiles.size();
     const long long units0 = (long long)F * p->tiles_per_f;
     if (units0 > 0x7fffffffLL / 64) {
@@ -205,7 +221,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
     const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK : corr::TC_ST;
     const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : corr::TC_MAX_SLICE;
-    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : p->sm_count;
+    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant == 2 ? p->sm_count / 2 : p->sm_count);
     const double per_sample = (path == CORR_PATH_DP4A) ? 40.0 : 8.0;  // cycles per time sample per unit
     const double epi = (path == CORR_PATH_DP4A) ? 1500.0 : 6000.0;    // cycles per unit, fixed
     const int min_slices = (T + max_slice - 1) / max_slice;
@@ -225,7 +241,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->t_per_slice = ((T + best_s - 1) / best_s + quantum - 1) / quantum * quantum;
     p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
     p->num_units = (int)(units0 * p->slices);
-    p->grid = (path == CORR_PATH_DP4A) ? p->num_units : std::min(p->num_units, p->sm_count);
+    p->grid = (path == CORR_PATH_DP4A) ? p->num_units
+              : (p->variant == 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
+                                  : std::min(p->num_units, p->sm_count);
     p->kernels_per_exec = 1;
     p->aligned = (N % 4 == 0) ? 1 : 0;
 
@@ -242,10 +260,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             corr_plan_destroy(p);
             return nullptr;
         }
-        if (cudaFuncSetAttribute(corr::corr_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 corr::TC_SMEM_BYTES) != cudaSuccess) {
-            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::TC_SMEM_BYTES,
-                    cudaGetErrorString(cudaGetLastError()));
+        cudaError_t e1 = cudaFuncSetAttribute(corr::corr_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              corr::TC_SMEM_BYTES);
+        cudaError_t e2 = cudaFuncSetAttribute(corr::corr_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              corr::T2_SMEM_BYTES);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) {
+            set_err("corr_plan_create: cannot reserve %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
+                    corr::T2_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
             return nullptr;
         }
@@ -261,11 +282,18 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
     const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
     const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
-    const cuuint32_t box[3] = {(cuuint32_t)corr::TC_BLK, 1u, (cuuint32_t)corr::TC_ST};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const int st = (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
+    const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS && p->variant == 2) {
+        const cuuint32_t boxy[3] = {64u, 1u, (cuuint32_t)st};  // half a y-block per CTA of the pair
+        r = get_encode_fn()(&p->tmap_y, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
+                            strides, boxy, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    }
     if (r != CUDA_SUCCESS) {
         set_err("cuTensorMapEncodeTiled failed with CUresult %d (N=%d F=%d T=%d)", (int)r, p->N, p->F, p->T);
         return CORR_ERR_CUDA;
@@ -314,18 +342,33 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     } else {
         int rc = build_tmap(p, packed_dev);
         if (rc != CORR_OK) return rc;
-        corr::TcParams prm;
-        prm.N = p->N;
-        prm.F = p->F;
-        prm.T = p->T;
-        prm.tiles_per_f = p->tiles_per_f;
-        prm.slices = p->slices;
-        prm.t_per_slice = p->t_per_slice;
-        prm.num_units = p->num_units;
-        prm.out_mode = out_mode;
-        prm.tiles = p->tiles_dev;
-        prm.vis = vis_dev;
-        corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
+        if (p->variant == 2) {
+            corr::Tc2Params prm;
+            prm.N = p->N;
+            prm.F = p->F;
+            prm.T = p->T;
+            prm.tiles_per_f = p->tiles_per_f;
+            prm.slices = p->slices;
+            prm.t_per_slice = p->t_per_slice;
+            prm.num_units = p->num_units;
+            prm.out_mode = out_mode;
+            prm.tiles = p->tiles_dev;
+            prm.vis = vis_dev;
+            corr::corr_tc2_kernel<<<p->grid, corr::T2_THREADS, corr::T2_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+        } else {
+            corr::TcParams prm;
+            prm.N = p->N;
+            prm.F = p->F;
+            prm.T = p->T;
+            prm.tiles_per_f = p->tiles_per_f;
+            prm.slices = p->slices;
+            prm.t_per_slice = p->t_per_slice;
+            prm.num_units = p->num_units;
+            prm.out_mode = out_mode;
+            prm.tiles = p->tiles_dev;
+            prm.vis = vis_dev;
+            corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
+        }
     }
     CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
     return CORR_OK;

@@ -44,14 +44,19 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Arrive on the barrier at the same smem offset in CTA `cta` of the cluster.
+// Arrive on the barrier at the same smem offset in CTA `cta` of the cluster.  Default
+// (release.cta) semantics on purpose: a .release.cluster arrive compiles to MEMBAR.ALL.GPU and a
+// .acquire.cluster wait to CCTL.IVALL (L1 invalidate) per poll, which tripled the stage time.  The
+// data these barriers guard never moves between SMs through a cache: each CTA writes its own
+// shared memory (made visible to the async proxy by fence.proxy.async) and the tensor core reads
+// it in place.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t cta)
 {
     asm volatile(
         "{\n\t"
         ".reg .b32 ra;\n\t"
         "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
-        "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t"
+        "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t"
         "}\n" ::"r"(bar), "r"(cta)
         : "memory");
 }
@@ -74,22 +79,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     while (!mbar_try_wait(bar, parity)) {
     }
 }
-// Cluster-scope acquire variant: used when the arrivals come from the peer CTA.
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
-{
-    uint32_t ok = 0;
-    while (!ok) {
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.b32 %0, 1, 0, p;\n\t"
-            "}\n"
-            : "=r"(ok)
-            : "r"(bar), "r"(parity)
-            : "memory");
-    }
-}
+// Wait on a barrier whose arrivals may come from the peer CTA (same default semantics, see above).
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) { mbar_wait(bar, parity); }
 
 // ---------------------------------------------------------------- proxies / fences
 // Generic-proxy smem writes (st.shared) -> visible to the async proxy (TMA, tcgen05.mma).

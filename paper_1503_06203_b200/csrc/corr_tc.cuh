@@ -308,6 +308,7 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         }
     }
 
+    __syncwarp();  // lanes that skipped the single-thread roles rejoin here
     ptx::tc_fence_before_sync();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc<1>(tmem, 512);

@@ -83,9 +83,9 @@ def test_split_t_and_multi_wave(corr, oracle):
     got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=123456)
     assert info["slices"] > 1
     assert np.array_equal(got, oracle.level1(packed))
-    packed = workloads.iid_gaussian(1024, 6, 300, seed=78)
+    packed = workloads.iid_gaussian(1024, 8, 300, seed=78)
     got, info = _run(corr, packed, corr.PATH_TCGEN05)
-    assert info["units"] > info["ctas"]
+    assert info["units"] > info["ctas"] // (2 if info["tile_x"] == 256 else 1)   # more than one wave
     assert np.array_equal(got, oracle.level1(packed))
 
 
