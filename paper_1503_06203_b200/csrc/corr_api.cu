@@ -15,6 +15,7 @@
 #include "corr_dp4a.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
+#include "corr_tc3.cuh"
 
 namespace {
 
@@ -85,7 +86,8 @@ struct corr_plan {
     // dp4a only
     int aligned;
     // tcgen05 only
-    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128 (corr_tc2.cuh)
+    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128, operands in smem
+                       // (corr_tc2.cuh); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default)
     CUtensorMap tmap;
     CUtensorMap tmap_y;
     const void *tmap_ptr;
@@ -117,7 +119,7 @@ int corr_plan_info(const corr_plan *p, int info[8])
         return CORR_ERR_INVALID_ARG;
     }
     info[0] = p->path;
-    info[1] = (p->variant == 2) ? 256 : p->tile;
+    info[1] = (p->variant >= 2) ? 256 : p->tile;
     info[2] = p->tile;
     info[3] = p->tiles_per_f;
     info[4] = p->slices;
@@ -196,11 +198,11 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->variant = 0;
     if (path == CORR_PATH_TCGEN05) {
         const char *v = getenv("CORR_TC_VARIANT");
-        p->variant = (v && !strcmp(v, "1")) ? 1 : 2;
+        p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : 3;
     }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
-    if (p->variant == 2) {
+    if (p->variant >= 2) {
         // pair tiles: x-block of 256 (two CTAs x 128), y-block of 128; keep those whose largest y
         // reaches their smallest x
         const int nbx = (N + 255) / 256;
@@ -219,9 +221,11 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     }
 
     // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
-    const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK : corr::TC_ST;
+    const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK
+                        : (p->variant == 3) ? corr::T3_ST * corr::T3_PL_STAGES  // tc3 runs whole groups of stages
+                                            : corr::TC_ST;
     const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : corr::TC_MAX_SLICE;
-    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant == 2 ? p->sm_count / 2 : p->sm_count);
+    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant >= 2 ? p->sm_count / 2 : p->sm_count);
     const double per_sample = (path == CORR_PATH_DP4A) ? 40.0 : 8.0;  // cycles per time sample per unit
     const double epi = (path == CORR_PATH_DP4A) ? 1500.0 : 6000.0;    // cycles per unit, fixed
     const int min_slices = (T + max_slice - 1) / max_slice;
@@ -242,7 +246,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
     p->num_units = (int)(units0 * p->slices);
     p->grid = (path == CORR_PATH_DP4A) ? p->num_units
-              : (p->variant == 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
+              : (p->variant >= 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
                                   : std::min(p->num_units, p->sm_count);
     p->kernels_per_exec = 1;
     p->aligned = (N % 4 == 0) ? 1 : 0;
@@ -264,9 +268,11 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
                                               corr::TC_SMEM_BYTES);
         cudaError_t e2 = cudaFuncSetAttribute(corr::corr_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::T2_SMEM_BYTES);
-        if (e1 != cudaSuccess || e2 != cudaSuccess) {
-            set_err("corr_plan_create: cannot reserve %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
-                    corr::T2_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
+        cudaError_t e3 = cudaFuncSetAttribute(corr::corr_tc3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              corr::T3_SMEM_BYTES);
+        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+            set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
+                    corr::T2_SMEM_BYTES, corr::T3_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
             return nullptr;
         }
@@ -283,12 +289,12 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
     const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const int st = (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
+    const int st = (p->variant == 3) ? corr::T3_ST : (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r == CUDA_SUCCESS && p->variant == 2) {
+    if (r == CUDA_SUCCESS && p->variant >= 2) {
         const cuuint32_t boxy[3] = {64u, 1u, (cuuint32_t)st};  // half a y-block per CTA of the pair
         r = get_encode_fn()(&p->tmap_y, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                             strides, boxy, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
@@ -342,7 +348,20 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     } else {
         int rc = build_tmap(p, packed_dev);
         if (rc != CORR_OK) return rc;
-        if (p->variant == 2) {
+        if (p->variant == 3) {
+            corr::Tc3Params prm;
+            prm.N = p->N;
+            prm.F = p->F;
+            prm.T = p->T;
+            prm.tiles_per_f = p->tiles_per_f;
+            prm.slices = p->slices;
+            prm.t_per_slice = p->t_per_slice;
+            prm.num_units = p->num_units;
+            prm.out_mode = out_mode;
+            prm.tiles = p->tiles_dev;
+            prm.vis = vis_dev;
+            corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+        } else if (p->variant == 2) {
             corr::Tc2Params prm;
             prm.N = p->N;
             prm.F = p->F;

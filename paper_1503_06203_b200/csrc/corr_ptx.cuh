@@ -176,6 +176,32 @@ __device__ __forceinline__ void mma_i8_ss(uint32_t d_tmem, uint64_t a_desc, uint
             : "memory");
 }
 
+// D[tmem] (+)= A[tmem] * B[smem desc]^T: the A operand is read from tensor memory (lane = row,
+// each 32-bit column = 4 consecutive K bytes; verified on B200 against a CPU product).
+template <int CG>
+__device__ __forceinline__ void mma_i8_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc,
+                                          uint32_t idesc, uint32_t accumulate)
+{
+    if constexpr (CG == 1)
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "setp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t"
+            "}\n" ::"r"(d_tmem),
+            "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+            : "memory");
+    else
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "setp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::2.kind::i8 [%0], [%1], %2, %3, p;\n\t"
+            "}\n" ::"r"(d_tmem),
+            "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+            : "memory");
+}
+
 // All prior tcgen05.mma of this thread arrive (once) on `bar` when they complete.
 template <int CG>
 __device__ __forceinline__ void mma_commit(uint32_t bar)
@@ -209,6 +235,34 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 __device__ __forceinline__ void tmem_ld_wait()
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// registers -> TMEM, 16 lanes x 128 bit, twice (8 columns): thread t writes r0 -> (lane t/4, col t%4),
+// r1 -> (lane t/4 + 8, col t%4), r2, r3 -> the same lanes, columns + 4.  The lane field of taddr
+// selects lanes [L, L+16) inside the warp's own lane quarter (L = 32*(warp%4) or + 16).
+__device__ __forceinline__ void tmem_st_16x128b_x2(uint32_t taddr, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3)
+{
+    asm volatile("tcgen05.st.sync.aligned.16x128b.x2.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r0), "r"(r1),
+                 "r"(r2), "r"(r3)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait()
+{
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+// Two transposed 16x16 byte matrices from shared memory: lanes 0-15 give the 16-byte row addresses
+// of matrix 0, lanes 16-31 those of matrix 1.  Measured on B200: thread t receives
+//   r0 = bytes (row 4(t%4)+0..3, column t/4) of matrix 0,   r1 = the same rows, column t/4 + 8,
+//   r2, r3 = the same of matrix 1
+// i.e. four ROW-consecutive bytes of one column per register: with rows = time samples and
+// columns = inputs this is exactly the tcgen05.st.16x128b fragment of a K-major A operand.
+__device__ __forceinline__ void ldsm_t_b8_x2(uint32_t saddr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3)
+{
+    asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(saddr)
+                 : "memory");
 }
 
 }  // namespace ptx

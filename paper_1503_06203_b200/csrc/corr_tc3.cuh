@@ -1,0 +1,344 @@
+// corr_tc3.cuh -- the large-N path (steps S1-S5) with the A operand in tensor memory.
+//
+// Same mathematics as corr_tc.cuh / corr_tc2.cuh (Eq. 1, summed over time
+// PAPER.md:48, upper triangle PAPER.md:50; x16 int8 operand planes, results shifted right by 8 in
+// the epilogue).  Same mapping as corr_tc2.cuh: two CTAs on the two SMs of one TPC form a cluster
+// and compute one 256 (x) by 128 (y) tile with tcgen05.mma.cta_group::2.
+//
+// What changed and why: ncu on corr_tc2_kernel (profiles/r01_tc2_ncu_summary.md) shows the
+// shared-memory data pipe at 93 % (LSU 60 % + tensor-core operand reads 33 %) with the tensor pipe at
+// 66 %: per 64-sample stage a CTA moved 256 + 96 + 192 wavefronts (plus replays) through a pipe
+// that carries 512 in the time the MMAs need.  Here the x-block planes never enter shared memory:
+//   * the unpack warps read the packed x-block with ldmatrix.m16n16.x2.trans.b8, which hands every
+//     thread four TIME-consecutive bytes of one input per register -- the transpose from the
+//     stream's element-contiguous order to the K-major order a TMEM operand needs, done by the
+//     load itself;
+//   * the planes 16*Re, 16*Im are formed in registers (3 logic ops per word) and written straight
+//     into TMEM with tcgen05.st.16x128b.x2, whose fragment is exactly the ldmatrix fragment;
+//   * the MMAs take A from TMEM ([a_tmem] form) and only B from shared memory.
+// Per stage and CTA: 128 (TC) + 96 (loads) + 64 (stores) wavefronts.
+//
+// Per CTA r (= rank in the pair) and per stage of 64 time samples:
+//   packed X_r  [64][128] bytes, 128-B swizzle   x in [256*bx2 + 128 r, +128)      (TMA)
+//   packed Yh_r [64][ 64] bytes,  64-B swizzle   y in [128*by + 64 r, +64)          (TMA)
+//   planes Bhr, Bhi [64][64] MN-major SW64 in shared memory (16*Re, 16*Im of the y-half)
+//   planes Ar, Ai in TMEM: lane = x - x0, 16 columns each = 64 K-bytes (2 K-steps of 32)
+// TMEM columns (per CTA, for its 128 x rows):
+//     0..127  IR += Ai * Br^T       128..255  Re += Ai * Bi^T + Ar * Br^T       256..383  RI += Ar * Bi^T
+//   384..511  A planes, 4 stages x (Ar 16 cols | Ai 16 cols)
+// column j of an accumulator <-> y = 128*by + j (j < 64 from CTA 0's y-half, j >= 64 from CTA 1's).
+//   Re = D[128 + j] >> 8,   Im = (D[j] - D[256 + j]) >> 8.
+//
+// Synchronisation across the pair: the packed ring (TMA -> unpack) is CTA-local.  The operand
+// ring (TMEM A stage + smem B stage, same index) is shared: unpack warps of BOTH CTAs arrive on the
+// leader's pl_full; the leader's MMA thread commits with multicast so pl_empty / acc_full fire in
+// both CTAs; epilogue warps of both CTAs arrive on the leader's acc_empty.
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "corr_dp4a.cuh"  // OutMode, baseline_index
+#include "corr_ptx.cuh"
+
+namespace corr {
+
+constexpr int T3_ST = 64;              // time samples per stage
+constexpr int T3_PK_STAGES = 6;        // packed-byte ring (covers TMA latency)
+constexpr int T3_PL_STAGES = 4;        // operand ring: TMEM A stage + smem B stage
+constexpr int T3_UNPACK_WARPS = 8;
+constexpr int T3_UNPACK_THREADS = 32 * T3_UNPACK_WARPS;
+constexpr int T3_EPI_WARP0 = 2 + T3_UNPACK_WARPS;
+constexpr int T3_EPI_WARPS = 4;
+constexpr int T3_THREADS = 32 * (T3_EPI_WARP0 + T3_EPI_WARPS);
+constexpr int T3_XBYTES = T3_ST * 128;             // packed x-block per stage
+constexpr int T3_YPLANE = T3_ST * 64;              // packed y-half / one y-half plane per stage
+constexpr int T3_PK_BYTES = T3_XBYTES + T3_YPLANE;
+constexpr int T3_PL_BYTES = 2 * T3_YPLANE;         // Bhr, Bhi
+constexpr int T3_EPI_PITCH = 16 * 8 + 8;
+constexpr int T3_EPI_BYTES = T3_EPI_WARPS * 32 * T3_EPI_PITCH;
+constexpr int T3_SMEM_BYTES = 1024 + T3_PK_STAGES * T3_PK_BYTES + T3_PL_STAGES * T3_PL_BYTES + T3_EPI_BYTES + 256;
+constexpr uint32_t T3_ACOL0 = 384;                 // first TMEM column of the A stages
+constexpr uint32_t T3_ACOLS = 32;                  // columns per A stage: Ar 16 | Ai 16
+
+struct Tc3Params {
+    int N, F, T;
+    int tiles_per_f;   // pair tiles (256 x 128) touching the upper triangle, per channel
+    int slices;
+    int t_per_slice;   // multiple of T3_ST
+    int num_units;     // F * tiles_per_f * slices
+    int out_mode;
+    const ushort2 *tiles;  // (bx2, by): x-block of 256, y-block of 128
+    int32_t *vis;
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
+corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ CUtensorMap tmap_y,
+                const Tc3Params p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *gbase = smem_raw + (base - ptx::smem_u32(smem_raw));
+    const uint32_t pk0 = base;
+    const uint32_t pl0 = pk0 + T3_PK_STAGES * T3_PK_BYTES;
+    const uint32_t epi0 = pl0 + T3_PL_STAGES * T3_PL_BYTES;
+    const uint32_t bar0 = epi0 + T3_EPI_BYTES;
+    uint8_t *epi_g = gbase + (epi0 - base);
+    auto pk_full = [&](int s) { return bar0 + 8u * s; };
+    auto pk_empty = [&](int s) { return bar0 + 8u * (T3_PK_STAGES + s); };
+    auto pl_full = [&](int s) { return bar0 + 8u * (2 * T3_PK_STAGES + s); };
+    auto pl_empty = [&](int s) { return bar0 + 8u * (2 * T3_PK_STAGES + T3_PL_STAGES + s); };
+    const uint32_t acc_full = bar0 + 8u * (2 * T3_PK_STAGES + 2 * T3_PL_STAGES);
+    const uint32_t acc_empty = acc_full + 8u;
+    const uint32_t tmem_slot = acc_empty + 8u;
+    volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + (tmem_slot - base));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = ptx::cluster_ctarank();  // 0 = leader (issues the MMAs)
+    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmap_x);
+        ptx::prefetch_tmap(&tmap_y);
+        for (int s = 0; s < T3_PK_STAGES; ++s) {
+            ptx::mbar_init(pk_full(s), 1);
+            ptx::mbar_init(pk_empty(s), T3_UNPACK_WARPS);
+        }
+        for (int s = 0; s < T3_PL_STAGES; ++s) {
+            ptx::mbar_init(pl_full(s), 2 * T3_UNPACK_WARPS);  // both CTAs' unpack warps (the leader's copy is used)
+            ptx::mbar_init(pl_empty(s), 1);
+        }
+        ptx::mbar_init(acc_full, 1);
+        ptx::mbar_init(acc_empty, 2 * T3_EPI_WARPS);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc<2>(tmem_slot, 512);
+        ptx::tmem_relinquish<2>();
+    }
+    ptx::tc_fence_before_sync();
+    ptx::cluster_sync();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot_g;
+    if (tmem != 0) __trap();  // all 512 columns were requested: the allocation starts at lane 0, column 0
+
+    const int units_per_f = p.tiles_per_f * p.slices;
+
+    if (warp == 0) {
+        // ===================== S1: TMA producer (each CTA loads its own blocks) =====================
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            for (int u = pair; u < p.num_units; u += npairs) {
+                const int f = u / units_per_f, rem = u % units_per_f;
+                const ushort2 tile = p.tiles[rem / p.slices];
+                const int slice = rem % p.slices;
+                const int t_begin = slice * p.t_per_slice;
+                const int t_end = min(p.T, t_begin + p.t_per_slice);
+                const int xc = tile.x * 256 + (int)rank * 128;
+                const int yc = tile.y * 128 + (int)rank * 64;
+                const int t_pad = t_begin + (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES) *
+                                                (T3_ST * T3_PL_STAGES);  // every unit runs whole groups of stages
+                for (int t = t_begin; t < t_pad; t += T3_ST) {
+                    ptx::mbar_wait(pk_empty(st), ph ^ 1u);
+                    ptx::mbar_arrive_expect_tx(pk_full(st), T3_PK_BYTES);
+                    const uint32_t dst = pk0 + st * T3_PK_BYTES;
+                    ptx::tma_load_3d(dst, &tmap_x, pk_full(st), xc, f, t);
+                    ptx::tma_load_3d(dst + T3_XBYTES, &tmap_y, pk_full(st), yc, f, t);
+                    if (++st == T3_PK_STAGES) { st = 0; ph ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== S4: MMA issuer (leader CTA only) =====================
+        // The whole warp runs this loop so that every operand is computed in warp-uniform code
+        // (uniform registers, no per-instruction ELECT / R2UR chains); one elected lane issues.
+        // Every unit runs a multiple of T3_PL_STAGES stages, so the stage index is a compile-time
+        // constant in the unrolled body and all descriptors are "uniform base + constant".
+        if (rank == 0) {
+            constexpr uint32_t idesc = make_idesc_i8(256, 128, true, true, /*A K-major (TMEM)*/ false, /*B MN-major*/ true);
+            uint32_t ph = 0, acc_ph = 0;
+            const bool issuer = ptx::elect_one();
+            for (int u = pair; u < p.num_units; u += npairs) {
+                const int rem = u % units_per_f;
+                const int slice = rem % p.slices;
+                const int t_begin = slice * p.t_per_slice;
+                const int t_end = min(p.T, t_begin + p.t_per_slice);
+                const int ngroups = (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES);
+                ptx::mbar_wait_cluster(acc_empty, acc_ph ^ 1u);
+                ptx::tc_fence_after_sync();
+                uint32_t acc = 0;
+                for (int g = 0; g < ngroups; ++g) {
+#pragma unroll
+                    for (int st = 0; st < T3_PL_STAGES; ++st) {
+                        ptx::mbar_wait_cluster(pl_full(st), ph);
+                        ptx::tc_fence_after_sync();
+                        if (issuer) {
+                            const uint32_t pl = pl0 + st * T3_PL_BYTES;
+                            const uint32_t a0 = T3_ACOL0 + (uint32_t)st * T3_ACOLS;  // TMEM base is 0 (checked at start)
+#pragma unroll
+                            for (int ks = 0; ks < T3_ST / 32; ++ks) {
+                                // B half per CTA: one 64-wide MN block, SW64, 8-row K groups 512 B apart; K-step = 2048 B
+                                const uint64_t dBr = make_smem_desc(pl + ks * 2048, T3_YPLANE, 512, 4);
+                                const uint64_t dBi = make_smem_desc(pl + T3_YPLANE + ks * 2048, T3_YPLANE, 512, 4);
+                                const uint32_t a_r = a0 + 8u * ks, a_i = a0 + 16u + 8u * ks;
+                                ptx::mma_i8_ts<2>(0, a_i, dBr, idesc, acc);    // IR
+                                ptx::mma_i8_ts<2>(128, a_i, dBi, idesc, acc);  // II  -> Re
+                                ptx::mma_i8_ts<2>(256, a_r, dBi, idesc, acc);  // RI
+                                ptx::mma_i8_ts<2>(128, a_r, dBr, idesc, 1);    // RR  -> Re
+                                acc = 1;
+                            }
+                            ptx::mma_commit_mcast2(pl_empty(st), 0x3);  // operand stage of BOTH CTAs is free
+                        }
+                        __syncwarp();
+                    }
+                    ph ^= 1u;
+                }
+                if (issuer) ptx::mma_commit_mcast2(acc_full, 0x3);
+                __syncwarp();
+                acc_ph ^= 1u;
+            }
+        }
+    } else if (warp < T3_EPI_WARP0) {
+        // ===================== S2: unpack =====================
+        const int ut = threadIdx.x - 64;
+        const int q = warp & 3;                 // TMEM lane quarter this warp may write: inputs 32q..32q+31
+        const int kh = (warp - 2) >> 2;         // which 32-sample half of the stage this warp transposes
+        // ldmatrix row address of this lane: matrix m = lane/16, row r = lane%16 -> sample 32 kh + 16 m + r
+        const int lrow = 32 * kh + 16 * (lane >> 4) + (lane & 15);
+        const uint32_t lds0 = (uint32_t)lrow * 128u + ((uint32_t)((2 * q + 0) ^ (lrow & 7)) << 4);
+        const uint32_t lds1 = (uint32_t)lrow * 128u + ((uint32_t)((2 * q + 1) ^ (lrow & 7)) << 4);
+        const int tbase = 32 * kh + 4 * (lane & 3);  // first sample of this thread's r0/r1 (r2/r3: + 16)
+        const uint32_t tdst = tmem + ((uint32_t)(32 * q) << 16) + T3_ACOL0 + 8u * kh;
+        int pst = 0, qst = 0;
+        uint32_t pph = 0, qph = 0;
+        for (int u = pair; u < p.num_units; u += npairs) {
+            const int rem = u % units_per_f;
+            const int slice = rem % p.slices;
+            const int t_begin = slice * p.t_per_slice;
+            const int t_end = min(p.T, t_begin + p.t_per_slice);
+            const int t_pad = t_begin + (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES) *
+                                            (T3_ST * T3_PL_STAGES);
+            for (int t = t_begin; t < t_pad; t += T3_ST) {
+                const int rows_valid = t_end - t;  // <= 0 in a padding stage: all-zero operands
+                // byte masks of this thread's four samples (zero beyond the slice)
+                uint32_t m0 = 0xF0F0F0F0u, m1 = 0xF0F0F0F0u;
+                if (rows_valid < T3_ST) {
+                    const int v0 = min(4, max(0, rows_valid - tbase)), v1 = min(4, max(0, rows_valid - tbase - 16));
+                    m0 = v0 ? (0xF0F0F0F0u >> (32 - 8 * v0)) : 0u;
+                    m1 = v1 ? (0xF0F0F0F0u >> (32 - 8 * v1)) : 0u;
+                }
+                ptx::mbar_wait(pk_full(pst), pph);
+                const uint32_t src = pk0 + pst * T3_PK_BYTES;
+                // ---- loads first: two transposing loads of the x-block, one 16-byte chunk of the y-half
+                uint32_t xa[4], xb[4];
+                ptx::ldsm_t_b8_x2(src + lds0, xa[0], xa[1], xa[2], xa[3]);   // inputs 32q + 0..15
+                ptx::ldsm_t_b8_x2(src + lds1, xb[0], xb[1], xb[2], xb[3]);   // inputs 32q + 16..31
+                const uint4 wy = *reinterpret_cast<const uint4 *>(gbase + (src - base) + T3_XBYTES + ut * 16);
+                ptx::mbar_wait_cluster(pl_empty(qst), qph ^ 1u);
+                // ---- A planes -> TMEM
+                const uint32_t ta = tdst + (uint32_t)qst * T3_ACOLS;
+                ptx::tmem_st_16x128b_x2(ta, (xa[0] ^ 0x80808080u) & m0, (xa[1] ^ 0x80808080u) & m0,
+                                        (xa[2] ^ 0x80808080u) & m1, (xa[3] ^ 0x80808080u) & m1);
+                ptx::tmem_st_16x128b_x2(ta + (16u << 16), (xb[0] ^ 0x80808080u) & m0, (xb[1] ^ 0x80808080u) & m0,
+                                        (xb[2] ^ 0x80808080u) & m1, (xb[3] ^ 0x80808080u) & m1);
+                ptx::tmem_st_16x128b_x2(ta + 16u, ((xa[0] << 4) ^ 0x80808080u) & m0, ((xa[1] << 4) ^ 0x80808080u) & m0,
+                                        ((xa[2] << 4) ^ 0x80808080u) & m1, ((xa[3] << 4) ^ 0x80808080u) & m1);
+                ptx::tmem_st_16x128b_x2(ta + (16u << 16) + 16u, ((xb[0] << 4) ^ 0x80808080u) & m0,
+                                        ((xb[1] << 4) ^ 0x80808080u) & m0, ((xb[2] << 4) ^ 0x80808080u) & m1,
+                                        ((xb[3] << 4) ^ 0x80808080u) & m1);
+                // ---- B planes -> shared memory, same physical offsets as the packed y-half
+                {
+                    uint8_t *dst = gbase + (pl0 - base) + qst * T3_PL_BYTES;
+                    const uint32_t off = (uint32_t)ut * 16u;
+                    const uint32_t m = ((int)(off >> 6) < rows_valid) ? 0xF0F0F0F0u : 0u;  // 64-B rows
+                    uint4 r, i;
+                    r.x = (wy.x ^ 0x80808080u) & m; r.y = (wy.y ^ 0x80808080u) & m;
+                    r.z = (wy.z ^ 0x80808080u) & m; r.w = (wy.w ^ 0x80808080u) & m;
+                    i.x = ((wy.x << 4) ^ 0x80808080u) & m; i.y = ((wy.y << 4) ^ 0x80808080u) & m;
+                    i.z = ((wy.z << 4) ^ 0x80808080u) & m; i.w = ((wy.w << 4) ^ 0x80808080u) & m;
+                    *reinterpret_cast<uint4 *>(dst + off) = r;
+                    *reinterpret_cast<uint4 *>(dst + T3_YPLANE + off) = i;
+                }
+                ptx::fence_proxy_async_smem();   // B planes: generic-proxy writes, read by the MMA's async proxy
+                ptx::tmem_st_wait();             // A planes are in TMEM
+                ptx::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) {
+                    ptx::mbar_arrive_cluster(pl_full(qst), 0);  // the leader's barrier
+                    ptx::mbar_arrive(pk_empty(pst));
+                }
+                if (++pst == T3_PK_STAGES) { pst = 0; pph ^= 1u; }
+                if (++qst == T3_PL_STAGES) { qst = 0; qph ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== S5: epilogue =====================
+        const int q = warp & 3;
+        uint8_t *stage = epi_g + (warp - T3_EPI_WARP0) * 32 * T3_EPI_PITCH;
+        const size_t Bn = (size_t)p.N * ((size_t)p.N + 1) / 2;
+        uint32_t acc_ph = 0;
+        for (int u = pair; u < p.num_units; u += npairs) {
+            const int f = u / units_per_f, rem = u % units_per_f;
+            const ushort2 tile = p.tiles[rem / p.slices];
+            const int x0 = tile.x * 256 + (int)rank * 128, y0 = tile.y * 128;
+            const int xw = x0 + q * 32;
+            ptx::mbar_wait_cluster(acc_full, acc_ph);
+            acc_ph ^= 1u;
+            ptx::tc_fence_after_sync();
+            const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+            for (int c = 0; c < 8; ++c) {
+                const int yc = y0 + c * 16;
+                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N);
+                if (!skip) {
+                    uint32_t ir[16], rr[16], ri[16];
+                    ptx::tmem_ld16(trow + c * 16, ir);
+                    ptx::tmem_ld16(trow + 128 + c * 16, rr);
+                    ptx::tmem_ld16(trow + 256 + c * 16, ri);
+                    ptx::tmem_ld_wait();
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int re = (int)rr[j] >> 8;
+                        const int im = (int)(ir[j] - ri[j]) >> 8;
+                        *reinterpret_cast<int2 *>(stage + lane * T3_EPI_PITCH + j * 8) = make_int2(re, im);
+                    }
+                    __syncwarp();
+                    const int cl = lane & 15;
+                    const int y = yc + cl;
+#pragma unroll 4
+                    for (int r2 = 0; r2 < 16; ++r2) {
+                        const int rl = r2 * 2 + (lane >> 4);
+                        const int x = xw + rl;
+                        if (x < p.N && y < p.N && x <= y) {
+                            const int2 v = *reinterpret_cast<const int2 *>(stage + rl * T3_EPI_PITCH + cl * 8);
+                            int32_t *o = p.vis + ((size_t)f * Bn + baseline_index(p.N, x, y)) * 2;
+                            if (p.out_mode == OUT_STORE) {
+                                *reinterpret_cast<int2 *>(o) = v;
+                            } else if (p.out_mode == OUT_RMW) {
+                                int2 old = *reinterpret_cast<int2 *>(o);
+                                old.x += v.x;
+                                old.y += v.y;
+                                *reinterpret_cast<int2 *>(o) = old;
+                            } else {
+                                atomicAdd(o, v.x);
+                                atomicAdd(o + 1, v.y);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                }
+            }
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
+        }
+    }
+
+    __syncwarp();  // lanes that skipped the single-thread roles rejoin here
+    ptx::tc_fence_before_sync();
+    ptx::cluster_sync();  // no CTA of the pair may exit while its peer still reads its smem / barriers
+    if (warp == 1) ptx::tmem_dealloc<2>(tmem, 512);
+}
+
+}  // namespace corr
