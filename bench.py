@@ -242,7 +242,7 @@ def main():
         "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
         "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
         "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
-        "kernel": "corr_tc_kernel", "kernel_ms": kernel_ms,
+        "kernel": "corr_tc3_kernel", "kernel_ms": kernel_ms,
         "algorithmic_ops_per_launch": eff_ops(N, F, T),
     }
     cpu_baseline = None

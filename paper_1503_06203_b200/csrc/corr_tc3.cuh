@@ -44,19 +44,19 @@
 namespace corr {
 
 constexpr int T3_ST = 64;              // time samples per stage
-constexpr int T3_PK_STAGES = 6;        // packed-byte ring (covers TMA latency)
+constexpr int T3_PK_STAGES = 5;        // packed-byte ring (covers TMA latency)
 constexpr int T3_PL_STAGES = 4;        // operand ring: TMEM A stage + smem B stage
 constexpr int T3_UNPACK_WARPS = 8;
 constexpr int T3_UNPACK_THREADS = 32 * T3_UNPACK_WARPS;
 constexpr int T3_EPI_WARP0 = 2 + T3_UNPACK_WARPS;
-constexpr int T3_EPI_WARPS = 4;
+constexpr int T3_EPI_WARPS = 8;             // two per TMEM lane quarter: column halves
 constexpr int T3_THREADS = 32 * (T3_EPI_WARP0 + T3_EPI_WARPS);
 constexpr int T3_XBYTES = T3_ST * 128;             // packed x-block per stage
 constexpr int T3_YPLANE = T3_ST * 64;              // packed y-half / one y-half plane per stage
 constexpr int T3_PK_BYTES = T3_XBYTES + T3_YPLANE;
 constexpr int T3_PL_BYTES = 2 * T3_YPLANE;         // Bhr, Bhi
-constexpr int T3_EPI_PITCH = 16 * 8 + 8;
-constexpr int T3_EPI_BYTES = T3_EPI_WARPS * 32 * T3_EPI_PITCH;
+constexpr int T3_EPI_PITCH = 128 * 8 + 16;        // one staged output row: 128 (Re,Im) pairs + parity slot
+constexpr int T3_EPI_BYTES = 128 * T3_EPI_PITCH;  // the CTA's whole 128 x 128 output block
 constexpr int T3_SMEM_BYTES = 1024 + T3_PK_STAGES * T3_PK_BYTES + T3_PL_STAGES * T3_PL_BYTES + T3_EPI_BYTES + 256;
 constexpr uint32_t T3_ACOL0 = 384;                 // first TMEM column of the A stages
 constexpr uint32_t T3_ACOLS = 32;                  // columns per A stage: Ar 16 | Ai 16
@@ -274,65 +274,86 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         }
     } else {
         // ===================== S5: epilogue =====================
+        // Eight warps: warp%4 = TMEM lane quarter q (hardware rule), h = column half.  Thread <-> output
+        // row x = x0 + 32 q + lane, columns y0 + 64 h .. + 63.  The accumulators are drained into a
+        // shared-memory image of the row (8 bytes per baseline, the layout of vis), TMEM is handed
+        // back to the MMA warp as soon as the last tcgen05.ld has completed, and the row segment
+        // leaves as ONE bulk copy (cp.async.bulk, or cp.reduce.async.bulk.add.s32 when the call
+        // accumulates) that overlaps the next unit's main loop.  Rows of the packed triangle start
+        // on 8-byte boundaries and bulk copies need 16: the row image is shifted by one slot when the
+        // global address is odd in 8-byte units, and at most one leading and one trailing baseline
+        // are written with ordinary stores.
         const int q = warp & 3;
-        uint8_t *stage = epi_g + (warp - T3_EPI_WARP0) * 32 * T3_EPI_PITCH;
-        const size_t Bn = (size_t)p.N * ((size_t)p.N + 1) / 2;
+        const int h = (warp - T3_EPI_WARP0) >> 2;
+        const int row = 32 * q + lane;
+        const uint32_t srow = epi0 + (uint32_t)row * T3_EPI_PITCH;
+        uint8_t *srow_g = epi_g + row * T3_EPI_PITCH;
+        const long long Bn = (long long)p.N * ((long long)p.N + 1) / 2;
+        const bool add = (p.out_mode != OUT_STORE);
         uint32_t acc_ph = 0;
         for (int u = pair; u < p.num_units; u += npairs) {
             const int f = u / units_per_f, rem = u % units_per_f;
             const ushort2 tile = p.tiles[rem / p.slices];
             const int x0 = tile.x * 256 + (int)rank * 128, y0 = tile.y * 128;
             const int xw = x0 + q * 32;
+            const int x = x0 + row;
+            // 8-byte index of (x, y0) in vis (formal when y0 < x: only its parity and offsets from it are used)
+            const long long g0 = (long long)f * Bn + (long long)x * p.N - (long long)x * (x - 1) / 2 - x + y0;
+            int2 *grow = reinterpret_cast<int2 *>(p.vis) + g0;
+            const uint32_t par = (uint32_t)(reinterpret_cast<uintptr_t>(grow) >> 3) & 1u;
+            ptx::bulk_wait_read0();  // this thread's previous row segment has left shared memory
             ptx::mbar_wait_cluster(acc_full, acc_ph);
             acc_ph ^= 1u;
             ptx::tc_fence_after_sync();
             const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
-#pragma unroll 1
-            for (int c = 0; c < 8; ++c) {
-                const int yc = y0 + c * 16;
-                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int col = 64 * h + 16 * c;
+                const int yc = y0 + col;
+                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N);  // warp-uniform
                 if (!skip) {
                     uint32_t ir[16], rr[16], ri[16];
-                    ptx::tmem_ld16(trow + c * 16, ir);
-                    ptx::tmem_ld16(trow + 128 + c * 16, rr);
-                    ptx::tmem_ld16(trow + 256 + c * 16, ri);
+                    ptx::tmem_ld16(trow + col, ir);
+                    ptx::tmem_ld16(trow + 128 + col, rr);
+                    ptx::tmem_ld16(trow + 256 + col, ri);
                     ptx::tmem_ld_wait();
+                    uint8_t *dst = srow_g + 8 * (par + col);
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         const int re = (int)rr[j] >> 8;
                         const int im = (int)(ir[j] - ri[j]) >> 8;
-                        *reinterpret_cast<int2 *>(stage + lane * T3_EPI_PITCH + j * 8) = make_int2(re, im);
+                        *reinterpret_cast<int2 *>(dst + j * 8) = make_int2(re, im);
                     }
-                    __syncwarp();
-                    const int cl = lane & 15;
-                    const int y = yc + cl;
-#pragma unroll 4
-                    for (int r2 = 0; r2 < 16; ++r2) {
-                        const int rl = r2 * 2 + (lane >> 4);
-                        const int x = xw + rl;
-                        if (x < p.N && y < p.N && x <= y) {
-                            const int2 v = *reinterpret_cast<const int2 *>(stage + rl * T3_EPI_PITCH + cl * 8);
-                            int32_t *o = p.vis + ((size_t)f * Bn + baseline_index(p.N, x, y)) * 2;
-                            if (p.out_mode == OUT_STORE) {
-                                *reinterpret_cast<int2 *>(o) = v;
-                            } else if (p.out_mode == OUT_RMW) {
-                                int2 old = *reinterpret_cast<int2 *>(o);
-                                old.x += v.x;
-                                old.y += v.y;
-                                *reinterpret_cast<int2 *>(o) = old;
-                            } else {
-                                atomicAdd(o, v.x);
-                                atomicAdd(o + 1, v.y);
-                            }
-                        }
-                    }
-                    __syncwarp();
                 }
             }
+            // TMEM is free for the next unit
             ptx::tc_fence_before_sync();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
+            // ---- write the row segment [jlo, jhi) of this thread
+            int jlo = max(64 * h, x - y0), jhi = min(64 * h + 64, p.N - y0);
+            if (x < p.N && jlo < jhi) {
+                ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
+                if ((par + jlo) & 1) {           // leading baseline on an odd 8-byte slot
+                    const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * (par + jlo));
+                    if (add) { atomicAdd(&grow[jlo].x, v.x); atomicAdd(&grow[jlo].y, v.y); }
+                    else grow[jlo] = v;
+                    ++jlo;
+                }
+                if ((jhi - jlo) & 1) {           // trailing baseline
+                    --jhi;
+                    const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * (par + jhi));
+                    if (add) { atomicAdd(&grow[jhi].x, v.x); atomicAdd(&grow[jhi].y, v.y); }
+                    else grow[jhi] = v;
+                }
+                if (jlo < jhi) {
+                    if (add) ptx::bulk_reduce_add_s32(grow + jlo, srow + 8u * (par + jlo), 8u * (jhi - jlo));
+                    else ptx::bulk_store(grow + jlo, srow + 8u * (par + jlo), 8u * (jhi - jlo));
+                }
+            }
+            ptx::bulk_commit();
         }
+        ptx::bulk_wait0();  // every row segment has been written before the CTA retires
     }
 
     __syncwarp();  // lanes that skipped the single-thread roles rejoin here
