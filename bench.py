@@ -31,6 +31,9 @@ if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
 METRIC = "effective correlation TOPS (8 ops/CMAC/baseline) at N=2048; % of int8 TC peak"
+# dram__bytes_read.sum + dram__bytes_write.sum of one corr_tc3_kernel launch on cfg3, from the ncu --set full
+# capture summarised in profiles/r01_tc3_ncu_summary.md (135.3 MB + 95.8 MB; algorithmic: 134.2 + 134.3 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = 231.1e6
 NOMINAL_INT8_TOPS = 4500.0  # dense int8 = 2x dense bf16 2250 (B200_PROFILING.md nominal table)
 
 
@@ -160,6 +163,7 @@ def main():
 
     import __graft_entry__
     import paper_1503_06203_b200 as corr
+    from paper_1503_06203_b200 import shard
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -203,10 +207,7 @@ def main():
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = shard.max_over_ranks(ms_total, dev)
     ms_per_step = ms_total / args.steps
     value = eff_ops(N, F, T) * world / (ms_per_step * 1e-3) / 1e12
 
@@ -220,10 +221,7 @@ def main():
         plan.execute_host(ph[i % 2], vh)   # synchronises the stream itself
     torch.cuda.synchronize(dev)
     e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = shard.max_over_ranks(e2e_s, dev)
     e2e_value = eff_ops(N, F, T) * world / e2e_s / 1e12
     checksum = int(vh.numpy()[0, :8, 0].astype(np.int64).sum())
 
@@ -238,7 +236,7 @@ def main():
     achieved = eff_ops(N, F, T) / (kernel_ms * 1e-3) / 1e12
     roofline = {
         "bound": "tensor", "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak,
-        "traffic": None,
+        "traffic": NCU_DRAM_BYTES_PER_LAUNCH if args.config == "cfg3" else None,
         "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
         "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
         "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
