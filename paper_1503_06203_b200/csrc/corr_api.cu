@@ -16,6 +16,7 @@
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
 #include "corr_tc3.cuh"
+#include "corr_tc4.cuh"
 
 namespace {
 
@@ -87,7 +88,9 @@ struct corr_plan {
     int aligned;
     // tcgen05 only
     int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128, operands in smem
-                       // (corr_tc2.cuh); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default)
+                       // (corr_tc2.cuh); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
+                       // 4: as 3 with three products per complex MAC (corr_tc4.cuh; CORR_TC_VARIANT=4)
+    int32_t *sums_dev; // variant 4: [2][slices][F][N] per-element sums of the stored bytes
     CUtensorMap tmap;
     CUtensorMap tmap_y;
     const void *tmap_ptr;
@@ -133,6 +136,7 @@ void corr_plan_destroy(corr_plan *p)
 {
     if (!p) return;
     if (p->tiles_dev) cudaFree(p->tiles_dev);
+    if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->packed_own) cudaFree(p->packed_own);
     if (p->vis_own) cudaFree(p->vis_own);
     delete p;
@@ -198,7 +202,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->variant = 0;
     if (path == CORR_PATH_TCGEN05) {
         const char *v = getenv("CORR_TC_VARIANT");
-        p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : 3;
+        p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : (v && !strcmp(v, "4")) ? 4 : 3;
     }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
@@ -222,9 +226,10 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
 
     // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
     const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK
-                        : (p->variant == 3) ? corr::T3_ST * corr::T3_PL_STAGES  // tc3 runs whole groups of stages
+                        : (p->variant == 4) ? corr::T4_GROUP
+                        : (p->variant == 3) ? corr::T3_ST * corr::T3_PL_STAGES  // tc3 / tc4 run whole groups of stages
                                             : corr::TC_ST;
-    const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : corr::TC_MAX_SLICE;
+    const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : (p->variant == 4) ? corr::T4_MAX_SLICE : corr::TC_MAX_SLICE;
     const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant >= 2 ? p->sm_count / 2 : p->sm_count);
     const double per_sample = (path == CORR_PATH_DP4A) ? 40.0 : 8.0;  // cycles per time sample per unit
     const double epi = (path == CORR_PATH_DP4A) ? 1500.0 : 6000.0;    // cycles per unit, fixed
@@ -248,7 +253,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->grid = (path == CORR_PATH_DP4A) ? p->num_units
               : (p->variant >= 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
                                   : std::min(p->num_units, p->sm_count);
-    p->kernels_per_exec = 1;
+    p->kernels_per_exec = (p->variant == 4) ? 2 : 1;  // tc4: corr_sums_kernel + corr_tc4_kernel
     p->aligned = (N % 4 == 0) ? 1 : 0;
 
     if (cudaMalloc(&p->tiles_dev, tiles.size() * sizeof(ushort2)) != cudaSuccess ||
@@ -270,6 +275,11 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
                                               corr::T2_SMEM_BYTES);
         cudaError_t e3 = cudaFuncSetAttribute(corr::corr_tc3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::T3_SMEM_BYTES);
+        if (e3 == cudaSuccess)
+            e3 = cudaFuncSetAttribute(corr::corr_tc4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      corr::T4_SMEM_BYTES);
+        if (e3 == cudaSuccess && p->variant == 4)
+            e3 = cudaMalloc(&p->sums_dev, 2 * (size_t)p->slices * F * N * sizeof(int32_t));
         if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
             set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
                     corr::T2_SMEM_BYTES, corr::T3_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
@@ -289,7 +299,7 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
     const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const int st = (p->variant == 3) ? corr::T3_ST : (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
+    const int st = (p->variant == 4) ? corr::T4_ST : (p->variant == 3) ? corr::T3_ST : (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -348,7 +358,30 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     } else {
         int rc = build_tmap(p, packed_dev);
         if (rc != CORR_OK) return rc;
-        if (p->variant == 3) {
+        if (p->variant == 4) {
+            // per-element sums of the stored bytes over every slice, then the 3-product kernel
+            const size_t nsum = (size_t)p->slices * p->F * p->N;
+            CUDA_TRY(cudaMemsetAsync(p->sums_dev, 0, 2 * nsum * sizeof(int32_t), stream), CORR_ERR_CUDA);
+            const int rows_per_block = corr::sums_rows_per_block(p->N);
+            dim3 sgrid((unsigned)((p->t_per_slice + rows_per_block - 1) / rows_per_block), (unsigned)p->F,
+                       (unsigned)p->slices);
+            corr::corr_sums_kernel<<<sgrid, corr::SUMS_THREADS, 0, stream>>>(packed_dev, p->sums_dev, p->sums_dev + nsum,
+                                                                             p->N, p->F, p->T, p->t_per_slice);
+            corr::Tc4Params prm;
+            prm.N = p->N;
+            prm.F = p->F;
+            prm.T = p->T;
+            prm.tiles_per_f = p->tiles_per_f;
+            prm.slices = p->slices;
+            prm.t_per_slice = p->t_per_slice;
+            prm.num_units = p->num_units;
+            prm.out_mode = out_mode;
+            prm.tiles = p->tiles_dev;
+            prm.sum_w = p->sums_dev;
+            prm.sum_lo = p->sums_dev + nsum;
+            prm.vis = vis_dev;
+            corr::corr_tc4_kernel<<<p->grid, corr::T4_THREADS, corr::T4_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+        } else if (p->variant == 3) {
             corr::Tc3Params prm;
             prm.N = p->N;
             prm.F = p->F;

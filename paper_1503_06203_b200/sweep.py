@@ -1,0 +1,68 @@
+"""N sweep of the X-engine (the x-axis of the paper's Fig. 4) and the five BASELINE.json
+shapes: effective TOPS and achieved HBM GB/s per shape, device-timed with CUDA events.
+
+    python -m paper_1503_06203_b200.sweep [--reps 20] [--csv out.csv]
+
+Inputs are random bytes generated on the device (every byte is a legal sample pair; timing does not
+depend on the values); correctness is the parity tests' job, not this script's.
+"""
+from __future__ import annotations
+
+import argparse
+import sys
+
+# (label, N, F, T, accumulate): sweep shapes keep the input >= 256 MB for small N so GB/s means something
+SHAPES = [
+    ("sweep", 16, 256, 65536, 0), ("sweep", 32, 128, 65536, 0), ("sweep", 64, 64, 65536, 0),
+    ("sweep", 128, 64, 32768, 0), ("sweep", 256, 32, 32768, 0), ("sweep", 512, 32, 16384, 0),
+    ("sweep", 1024, 16, 16384, 0), ("sweep", 2048, 8, 16384, 0), ("sweep", 4096, 4, 8192, 0),
+    ("sweep", 8192, 1, 8192, 0),
+    ("cfg1", 16, 4, 1024, 0), ("cfg2", 256, 16, 16384, 0), ("cfg3", 2048, 8, 8192, 0),
+    ("cfg4", 8192, 1, 4096, 0), ("cfg5 (one accumulate call)", 512, 64, 8192, 1),
+]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--reps", type=int, default=20)
+    ap.add_argument("--csv", default=None)
+    args = ap.parse_args()
+    import torch
+    from . import Plan
+    if not torch.cuda.is_available():
+        sys.exit("sweep needs a CUDA device (there is no CPU path)")
+    dev = torch.device("cuda:0")
+    rows = []
+    for label, N, F, T, acc in SHAPES:
+        plan = Plan(N, F, T)
+        nbuf = 2 if N * F * T >= (64 << 20) else 8
+        ins = [torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device=dev) for _ in range(nbuf)]
+        vis = torch.zeros((F, plan.baselines, 2), dtype=torch.int32, device=dev)
+        for i in range(3):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(args.reps):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.reps
+        ops = 8.0 * plan.baselines * F * T
+        out_bytes = vis.numel() * 4 * (2 if acc else 1)
+        gbs = (N * F * T + out_bytes) / (ms * 1e-3) / 1e9
+        rows.append((label, N, F, T, plan.info["path"], plan.info["slices"], plan.info["units"], ms,
+                     ops / (ms * 1e-3) / 1e12, gbs))
+        plan.close()
+        del ins, vis
+        torch.cuda.empty_cache()
+    hdr = ("shape", "N", "F", "T", "path", "slices", "units", "ms", "eff_TOPS", "HBM_GBs")
+    lines = [",".join(hdr)] + [",".join(f"{v:.4g}" if isinstance(v, float) else str(v) for v in r) for r in rows]
+    print("\n".join(lines))
+    if args.csv:
+        with open(args.csv, "w") as fh:
+            fh.write("\n".join(lines) + "\n")
+
+
+if __name__ == "__main__":
+    main()

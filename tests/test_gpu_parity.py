@@ -115,6 +115,26 @@ def test_determinism(corr):
     assert np.array_equal(r1, r3)
 
 
+@pytest.mark.parametrize("variant", ["1", "2", "3", "4"])
+def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
+    # CORR_TC_VARIANT selects the kernel at plan creation: 1 single-CTA tiles, 2 CTA pair with both
+    # operands in shared memory, 3 A operand in TMEM (default), 4 three products per complex MAC
+    # (offset route, Eq. 3).  Same bits from all of them, including ragged N, split T and accumulation.
+    monkeypatch.setenv("CORR_TC_VARIANT", variant)
+    for (N, F, T, seed) in [(272, 3, 1000, 11), (1024, 2, 333, 12), (256, 1, 40000, 13), (2048, 1, 640, 14)]:
+        packed = workloads.uniform_bytes(N, F, T, seed=seed)
+        want = oracle.level1(packed)
+        got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=-559038737)
+        assert np.array_equal(got, want), (variant, N, F, T)
+        again, _ = _run(corr, packed, corr.PATH_TCGEN05, accumulate_into=got.copy())
+        assert np.array_equal(again, 2 * want), (variant, N, F, T, "accumulate")
+    # extreme values: all samples -8-8i (largest magnitudes everywhere) and the 0xFF byte (+7+7i)
+    for byte in (0x00, 0xFF, 0x0F, 0xF0):
+        packed = np.full((4096, 2, 256), byte, np.uint8)
+        got, _ = _run(corr, packed, corr.PATH_TCGEN05)
+        assert np.array_equal(got, oracle.level1(packed)), (variant, hex(byte))
+
+
 def test_execute_host(corr, oracle):
     import torch
     packed = workloads.iid_gaussian(160, 2, 700, seed=9)
