@@ -60,7 +60,8 @@ enum {
 enum {
     CORR_PATH_AUTO = 0,  /* library chooses from (N, F, T) */
     CORR_PATH_DP4A = 1,  /* CUDA-core dp4a kernels; any N (small-N path) */
-    CORR_PATH_TCGEN05 = 2 /* TMA + tcgen05 int8 MMA, int32 accumulators in TMEM; needs N % 16 == 0 */
+    CORR_PATH_TCGEN05 = 2, /* TMA + tcgen05 int8 MMA, int32 accumulators in TMEM; needs N % 16 == 0 */
+    CORR_PATH_IMMA = 3     /* TMA + warp-level int8 MMA on whole channels; N = 16, 32 or 64 (small-N path) */
 };
 
 /* corr_plan_create -- validate the shape, choose the path, build the triangular tile schedule
@@ -110,7 +111,7 @@ size_t corr_vis_elems(const corr_plan *plan);          /* F * N(N+1)/2 * 2 int32
 size_t corr_baseline_index(int N, int x, int y);       /* b(x,y); requires 0 <= x <= y < N, else (size_t)-1 */
 
 /* Plan introspection (host only).  Writes up to 8 ints:
- *   info[0] path actually chosen (CORR_PATH_DP4A / CORR_PATH_TCGEN05)
+ *   info[0] path actually chosen (CORR_PATH_DP4A / CORR_PATH_TCGEN05 / CORR_PATH_IMMA)
  *   info[1] tile edge in elements along x     info[2] tile edge along y
  *   info[3] tiles per channel on or above the diagonal
  *   info[4] T-slices per tile (split-T factor) info[5] total work units = F*tiles*slices

@@ -7,7 +7,7 @@ from pathlib import Path
 _HERE = Path(__file__).resolve().parent
 _LIB_PATH = _HERE / "libcorr_b200.so"
 
-PATH_AUTO, PATH_DP4A, PATH_TCGEN05 = 0, 1, 2
+PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",

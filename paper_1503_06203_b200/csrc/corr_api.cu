@@ -13,6 +13,7 @@
 
 #include "../../include/corr.h"
 #include "corr_dp4a.cuh"
+#include "corr_imma.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
 #include "corr_tc3.cuh"
@@ -152,7 +153,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         set_err("corr_plan_create: N=%d too large for the tile table", N);
         return nullptr;
     }
-    if (path != CORR_PATH_AUTO && path != CORR_PATH_DP4A && path != CORR_PATH_TCGEN05) {
+    if (path != CORR_PATH_AUTO && path != CORR_PATH_DP4A && path != CORR_PATH_TCGEN05 && path != CORR_PATH_IMMA) {
         set_err("corr_plan_create: unknown path %d", path);
         return nullptr;
     }
@@ -174,8 +175,16 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             path = CORR_PATH_DP4A;
         else if (force && !strcmp(force, "tcgen05"))
             path = CORR_PATH_TCGEN05;
+        else if (force && !strcmp(force, "imma"))
+            path = CORR_PATH_IMMA;
         else
-            path = (N % 16 == 0 && N >= 96) ? CORR_PATH_TCGEN05 : CORR_PATH_DP4A;
+            path = (N == 16 || N == 32 || N == 64) ? CORR_PATH_IMMA
+                   : (N % 16 == 0 && N >= 96)      ? CORR_PATH_TCGEN05
+                                                   : CORR_PATH_DP4A;
+    }
+    if (path == CORR_PATH_IMMA && !(N == 16 || N == 32 || N == 64)) {
+        set_err("corr_plan_create: the warp-MMA path takes N = 16, 32 or 64, got N=%d", N);
+        return nullptr;
     }
     if (path == CORR_PATH_TCGEN05 && N % 16 != 0) {
         set_err("corr_plan_create: the tcgen05 path needs N %% 16 == 0 (TMA row stride), got N=%d", N);
@@ -193,6 +202,34 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->T = T;
     p->path = path;
     p->sm_count = prop.multiProcessorCount;
+
+    if (path == CORR_PATH_IMMA) {
+        // whole channels per CTA: strips of 128/N channels x chunks of time samples (corr_imma.cuh)
+        if (!get_encode_fn()) {
+            set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
+            delete p;
+            return nullptr;
+        }
+        const int fb = 128 / N;
+        const int strips = (F + fb - 1) / fb;
+        int chunks = std::max(1, std::min((2 * p->sm_count + strips - 1) / strips, T / 512));
+        p->t_per_slice = ((T + chunks - 1) / chunks + corr::IM_ROWS - 1) / corr::IM_ROWS * corr::IM_ROWS;
+        p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
+        p->tile = N;
+        p->tiles_per_f = 1;
+        p->num_units = strips * p->slices;
+        p->grid = p->num_units;
+        p->kernels_per_exec = 1;
+        cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e != cudaSuccess) {
+            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::IM_SMEM_BYTES, cudaGetErrorString(e));
+            delete p;
+            return nullptr;
+        }
+        return p;
+    }
 
     // ---- S3: the triangular tile table (only tiles on or above the diagonal)
     if (path == CORR_PATH_DP4A)
@@ -295,6 +332,22 @@ corr_plan *corr_plan_create(int N, int F, int T) { return corr_plan_create_ex(N,
 static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
 {
     if (p->tmap_ptr == packed_dev) return CORR_OK;
+    if (p->path == CORR_PATH_IMMA) {
+        // packed[T][F][N] as a byte matrix, innermost first: (F*N, T), row stride F*N bytes
+        const cuuint64_t dims2[2] = {(cuuint64_t)p->F * (cuuint64_t)p->N, (cuuint64_t)p->T};
+        const cuuint64_t strides2[1] = {(cuuint64_t)p->F * (cuuint64_t)p->N};
+        const cuuint32_t box2[2] = {128u, (cuuint32_t)corr::IM_ROWS};
+        const cuuint32_t estr2[2] = {1u, 1u};
+        CUresult r2 = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(packed_dev), dims2,
+                                      strides2, box2, estr2, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r2 != CUDA_SUCCESS) {
+            set_err("cuTensorMapEncodeTiled (2-D) failed with CUresult %d (N=%d F=%d T=%d)", (int)r2, p->N, p->F, p->T);
+            return CORR_ERR_CUDA;
+        }
+        p->tmap_ptr = packed_dev;
+        return CORR_OK;
+    }
     // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
     const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
     const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
@@ -339,7 +392,24 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         out_mode = accumulate_flag ? corr::OUT_RMW : corr::OUT_STORE;
     }
 
-    if (p->path == CORR_PATH_DP4A) {
+    if (p->path == CORR_PATH_IMMA) {
+        int rc = build_tmap(p, packed_dev);
+        if (rc != CORR_OK) return rc;
+        corr::ImmaParams prm;
+        prm.N = p->N;
+        prm.F = p->F;
+        prm.T = p->T;
+        prm.t_per_chunk = p->t_per_slice;
+        prm.out_mode = out_mode;
+        prm.vis = vis_dev;
+        dim3 grid((unsigned)(p->num_units / p->slices), (unsigned)p->slices);
+        if (p->N == 16)
+            corr::corr_imma_kernel<1><<<grid, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
+        else if (p->N == 32)
+            corr::corr_imma_kernel<2><<<grid, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
+        else
+            corr::corr_imma_kernel<4><<<grid, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
+    } else if (p->path == CORR_PATH_DP4A) {
         dim3 grid((unsigned)(p->F * p->tiles_per_f), (unsigned)p->slices);
         switch (p->tile) {
         case 16:

@@ -1,0 +1,229 @@
+// corr_imma.cuh -- step S4' of the hot path for N = 16, 32, 64: warp-level int8 tensor-core
+// MMA (mma.sync.m16n8k32.s8) on whole channels, fed by TMA.
+//
+// Why not dp4a here: measured on B200, IDP.4A issues 64 lanes/clk/SM = 17.5 T dp4a/s, i.e. 140
+// effective TOPS at one dp4a per complex MAC, while streaming N = 16 inputs at HBM speed needs
+// 4 (N + 1) ops per byte x 6.5 TB/s = 440 effective TOPS.  The legacy warp-level IMMA path
+// measures 1146 TOPS, enough to stay memory-bound up to N = 32 (corr_dp4a.cuh remains the path
+// for every other small N).  The paper makes the small-N observation for its own tiles at
+// PAPER.md:72; the result computed is Eq. 1 summed over time on the
+// upper triangle.
+//
+// Data movement.  The stream [T][F][N] is a plain 2-D byte matrix with rows of F*N bytes, so a CTA
+// takes a 128-byte-wide column strip (FB = 128/N whole channels) and a chunk of time samples:
+// TMA boxes [128 t][128 B] with 128-byte swizzle into a ring of stages.
+//
+// Arithmetic.  ldmatrix.m16n16.trans.b8 hands every thread four TIME-consecutive bytes of one
+// input, which is both the A fragment (rows = inputs 16mt..16mt+15, K = 32 samples) and, split in
+// halves, the B fragments (columns = inputs 8nt..8nt+7) of mma.m16n8k32.  Planes 16*Re =
+// (w ^ 0x80) & 0xF0 and 16*Im = ((w << 4) ^ 0x80) & 0xF0 are exact int8; per 32 samples
+//     Re[mt][nt] += Pr[mt] Pr[nt]^T + Pi[mt] Pi[nt]^T      only blocks with nt >= 2 mt (upper triangle)
+//     IR[mt][nt] += Pi[mt] Pr[nt]^T                         all blocks
+// and at the end  Re >> 8,  Im[x][y] = (IR[x][y] - IR[y][x]) >> 8  (sum Re[x] Im[y] = IR[y][x]).
+// Three MMAs per block pair instead of four because the whole channel is in one CTA.
+//
+// Warps: one per (channel of the strip, m-tile set, K-split); partial sums of the K-split warps
+// are combined with shared-memory atomics in the ring's memory after the pipeline has drained,
+// then written with store / read-add-store / atomicAdd like the other paths.
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "corr_dp4a.cuh"  // OutMode, baseline_index
+#include "corr_ptx.cuh"
+
+namespace corr {
+
+constexpr int IM_ROWS = 128;                 // time samples per stage
+constexpr int IM_STAGE_BYTES = IM_ROWS * 128;
+constexpr int IM_STAGES = 6;
+constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 256;
+
+template <int NT16> struct ImmaCfg {
+    static constexpr int N = 16 * NT16;
+    static constexpr int FB = 128 / N;                         // channels per strip
+    static constexpr int MS = (NT16 == 4) ? 2 : 1;             // m-tile sets per channel
+    static constexpr int KS = (NT16 == 1) ? 2 : (NT16 == 2) ? 4 : 2;   // K-split
+    static constexpr int WARPS = FB * MS * KS;                 // consumer warps (16, 16, 8)
+    static constexpr int THREADS = 32 * (WARPS + 1);           // + the TMA producer warp
+};
+
+struct ImmaParams {
+    int N, F, T;
+    int t_per_chunk;   // multiple of 32
+    int out_mode;
+    int32_t *vis;
+};
+
+__device__ __forceinline__ void mma_s8(int (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// One K-block (32 samples): the products of m-tile MT (accumulator set S of this warp) with every n-tile.
+template <int NT16, int MT, int S>
+__device__ __forceinline__ void imma_mtile(const uint32_t (&pr)[NT16][4], const uint32_t (&pi)[NT16][4],
+                                           int (&re)[2][2 * NT16][4], int (&ir)[2][2 * NT16][4])
+{
+#pragma unroll
+    for (int nt = 0; nt < 2 * NT16; ++nt) {
+        const int bs = nt >> 1, h = nt & 1;   // source m-tile and half of the B fragment
+        mma_s8(ir[S][nt], pi[MT], pr[bs][h], pr[bs][2 + h]);
+        if (nt >= 2 * MT) {                   // blocks that touch the upper triangle
+            mma_s8(re[S][nt], pr[MT], pr[bs][h], pr[bs][2 + h]);
+            mma_s8(re[S][nt], pi[MT], pi[bs][h], pi[bs][2 + h]);
+        }
+    }
+}
+
+template <int NT16>
+__global__ void __launch_bounds__(ImmaCfg<NT16>::THREADS, 1)
+corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
+{
+    using C = ImmaCfg<NT16>;
+    constexpr int N = C::N;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *gbase = smem_raw + (base - ptx::smem_u32(smem_raw));
+    const uint32_t bar0 = base + IM_STAGES * IM_STAGE_BYTES;
+    auto full = [&](int s) { return bar0 + 8u * s; };
+    auto empty = [&](int s) { return bar0 + 8u * (IM_STAGES + s); };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int strip = blockIdx.x, chunk = blockIdx.y;
+    const int t_begin = chunk * p.t_per_chunk;
+    const int t_end = min(p.T, t_begin + p.t_per_chunk);
+    const int nstages = (t_end - t_begin + IM_ROWS - 1) / IM_ROWS;
+
+    if (threadIdx.x == 0) {
+        ptx::prefetch_tmap(&tmap);
+        for (int s = 0; s < IM_STAGES; ++s) {
+            ptx::mbar_init(full(s), 1);
+            ptx::mbar_init(empty(s), C::WARPS);
+        }
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();
+
+    // accumulators of this warp: up to two m-tiles x all n-tiles, (16 x 8 int32 per block) / 32 lanes
+    int re[2][2 * NT16][4], ir[2][2 * NT16][4];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int nt = 0; nt < 2 * NT16; ++nt)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) re[s][nt][j] = ir[s][nt][j] = 0;
+
+    const int ch = warp % C::FB;                    // channel inside the strip
+    const int ms = (warp / C::FB) % C::MS;          // m-tile set
+    const int ks = warp / (C::FB * C::MS);          // K-split index
+    const int f = strip * C::FB + ch;
+
+    if (warp == C::WARPS) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            for (int it = 0; it < nstages; ++it) {
+                const int s = it % IM_STAGES;
+                ptx::mbar_wait(empty(s), ((uint32_t)(it / IM_STAGES) & 1u) ^ 1u);
+                ptx::mbar_arrive_expect_tx(full(s), IM_STAGE_BYTES);
+                ptx::tma_load_2d(base + s * IM_STAGE_BYTES, &tmap, full(s), strip * 128, t_begin + it * IM_ROWS);
+            }
+        }
+    } else {
+        // ===================== consumers =====================
+        const uint32_t c16 = (uint32_t)(ch * N) >> 4;   // first 16-byte chunk of this channel in a 128-byte row
+        for (int it = 0; it < nstages; ++it) {
+            const int s = it % IM_STAGES;
+            ptx::mbar_wait(full(s), (uint32_t)(it / IM_STAGES) & 1u);
+            const uint32_t stage = base + s * IM_STAGE_BYTES;
+            if (f < p.F) {
+#pragma unroll
+                for (int kk = 0; kk < IM_ROWS / 32 / C::KS; ++kk) {
+                    const int kb = ks + C::KS * kk;                       // K-block of 32 samples inside the stage
+                    const int valid = t_end - (t_begin + it * IM_ROWS + 32 * kb);   // samples of this K-block inside the chunk
+                    if (valid <= 0) continue;
+                    const uint32_t r = 32u * kb + lane;                   // ldmatrix row of this lane (time sample)
+                    uint32_t pr[NT16][4], pi[NT16][4];
+#pragma unroll
+                    for (int mt = 0; mt < NT16; ++mt) {
+                        uint32_t w[4];
+                        ptx::ldsm_t_b8_x2(stage + r * 128u + (((c16 + mt) ^ (r & 7u)) << 4), w[0], w[1], w[2], w[3]);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            pr[mt][j] = (w[j] ^ 0x80808080u) & 0xF0F0F0F0u;
+                            pi[mt][j] = ((w[j] << 4) ^ 0x80808080u) & 0xF0F0F0F0u;
+                        }
+                    }
+                    if (valid < 32) {   // ragged end of the chunk: zero the samples beyond it (registers 0,1: 4c.., 2,3: 16+4c..)
+                        const int c4 = 4 * (lane & 3);
+                        const int v0 = min(4, max(0, valid - c4)), v1 = min(4, max(0, valid - c4 - 16));
+                        const uint32_t m0 = v0 ? (0xFFFFFFFFu >> (32 - 8 * v0)) : 0u;
+                        const uint32_t m1 = v1 ? (0xFFFFFFFFu >> (32 - 8 * v1)) : 0u;
+#pragma unroll
+                        for (int mt = 0; mt < NT16; ++mt) {
+                            pr[mt][0] &= m0; pr[mt][1] &= m0; pr[mt][2] &= m1; pr[mt][3] &= m1;
+                            pi[mt][0] &= m0; pi[mt][1] &= m0; pi[mt][2] &= m1; pi[mt][3] &= m1;
+                        }
+                    }
+                    if constexpr (NT16 == 4) {
+                        if (ms == 0) { imma_mtile<4, 0, 0>(pr, pi, re, ir); imma_mtile<4, 3, 1>(pr, pi, re, ir); }
+                        else         { imma_mtile<4, 1, 0>(pr, pi, re, ir); imma_mtile<4, 2, 1>(pr, pi, re, ir); }
+                    } else if constexpr (NT16 == 2) {
+                        imma_mtile<2, 0, 0>(pr, pi, re, ir); imma_mtile<2, 1, 1>(pr, pi, re, ir);
+                    } else {
+                        imma_mtile<1, 0, 0>(pr, pi, re, ir);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(empty(s));
+        }
+    }
+
+    // ---- combine the K-split warps in shared memory (the ring is drained: every stage was consumed)
+    __syncthreads();
+    int *red = reinterpret_cast<int *>(gbase);          // [FB][2][N*N]: Re, IR
+    for (int i = threadIdx.x; i < C::FB * 2 * N * N; i += C::THREADS) red[i] = 0;
+    __syncthreads();
+    if (warp < C::WARPS && f < p.F) {
+        int *rre = red + (ch * 2 + 0) * N * N, *rir = red + (ch * 2 + 1) * N * N;
+        const int g = lane >> 2, c2 = 2 * (lane & 3);
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            int mt;
+            if (NT16 == 4) mt = (ms == 0) ? (s == 0 ? 0 : 3) : (s == 0 ? 1 : 2);
+            else mt = s;
+            if (mt >= NT16) continue;
+#pragma unroll
+            for (int nt = 0; nt < 2 * NT16; ++nt) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int x = 16 * mt + g + 8 * (j >> 1), y = 8 * nt + c2 + (j & 1);
+                    atomicAdd(&rir[x * N + y], ir[s][nt][j]);
+                    if (nt >= 2 * mt) atomicAdd(&rre[x * N + y], re[s][nt][j]);
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- S5: form (Re, Im), keep x <= y, write
+    const size_t B = (size_t)N * (N + 1) / 2;
+    for (int i = threadIdx.x; i < C::FB * N * N; i += C::THREADS) {
+        const int c = i / (N * N), x = (i / N) % N, y = i % N;
+        const int fo = strip * C::FB + c;
+        if (fo >= p.F || y < x) continue;
+        const int *rre = red + (c * 2 + 0) * N * N, *rir = red + (c * 2 + 1) * N * N;
+        const int vre = rre[x * N + y] >> 8;
+        const int vim = (rir[x * N + y] - rir[y * N + x]) >> 8;
+        int32_t *o = p.vis + 2 * ((size_t)fo * B + baseline_index(N, x, y));
+        if (p.out_mode == OUT_STORE) { o[0] = vre; o[1] = vim; }
+        else if (p.out_mode == OUT_RMW) { o[0] += vre; o[1] += vim; }
+        else { atomicAdd(o, vre); atomicAdd(o + 1, vim); }
+    }
+}
+
+}  // namespace corr

@@ -65,6 +65,35 @@ def test_tcgen05_small_shapes(corr, oracle, N):
             assert np.array_equal(got, oracle.level1(packed)), (N, F, T)
 
 
+@pytest.mark.parametrize("N", [16, 32, 64])
+def test_imma_small_n(corr, oracle, N):
+    # warp-MMA path (whole channels per CTA): ragged T, F not a multiple of the channels per strip,
+    # several time chunks (atomic accumulation), stale output, accumulate flag, extreme bytes
+    for F in (1, 3, 9):
+        for T in TINY_T + [1000, 4099]:
+            packed = workloads.uniform_bytes(N, F, T, seed=N * 31337 + F * 31 + T)
+            got, info = _run(corr, packed, corr.PATH_IMMA, prefill=-559038737)
+            assert info["path"] == corr.PATH_IMMA
+            assert np.array_equal(got, oracle.level1(packed)), (N, F, T)
+    packed = workloads.iid_gaussian(N, 5, 70000, seed=N)          # several chunks per channel
+    want = oracle.level1(packed)
+    got, info = _run(corr, packed, corr.PATH_IMMA, prefill=123)
+    assert info["slices"] > 1
+    assert np.array_equal(got, want)
+    again, _ = _run(corr, packed, corr.PATH_IMMA, accumulate_into=got.copy())
+    assert np.array_equal(again, 2 * want)
+    small = workloads.uniform_bytes(N, 2, 300, seed=7)             # one chunk: read-add-store
+    w2 = oracle.level1(small)
+    acc, info = _run(corr, small, corr.PATH_IMMA, accumulate_into=w2.copy())
+    assert info["slices"] == 1 and np.array_equal(acc, 2 * w2)
+    for byte in (0x00, 0xFF, 0x0F, 0xF0):
+        packed = np.full((5000, 3, N), byte, np.uint8)
+        got, _ = _run(corr, packed, corr.PATH_IMMA)
+        assert np.array_equal(got, oracle.level1(packed)), (N, hex(byte))
+    auto, info = _run(corr, small)                                  # AUTO picks this path for N = 16, 32, 64
+    assert info["path"] == corr.PATH_IMMA and np.array_equal(auto, w2)
+
+
 def test_tcgen05_extreme_values(corr, oracle):
     # all samples -8-8i: largest products (16*-8 = -128 on both operands), Re = 128 T, Im = 0
     N, F, T = 256, 2, 4096
@@ -113,6 +142,9 @@ def test_determinism(corr):
     assert np.array_equal(r1, r2)
     r3, _ = _run(corr, packed, corr.PATH_DP4A)
     assert np.array_equal(r1, r3)
+    packed = workloads.iid_gaussian(64, 7, 3000, seed=6)
+    assert np.array_equal(_run(corr, packed, corr.PATH_IMMA)[0], _run(corr, packed, corr.PATH_DP4A)[0])
+    assert np.array_equal(_run(corr, packed, corr.PATH_IMMA)[0], _run(corr, packed, corr.PATH_TCGEN05)[0])
 
 
 @pytest.mark.parametrize("variant", ["1", "2", "3", "4"])
@@ -155,6 +187,8 @@ def test_invalid_arguments(corr):
             corr.corr_plan_create(*bad)
     with pytest.raises(corr.CorrError):
         corr.corr_plan_create(100, 1, 64, corr.PATH_TCGEN05)   # N % 16 != 0
+    with pytest.raises(corr.CorrError):
+        corr.corr_plan_create(48, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N = 16, 32, 64 only
 
 
 # ------------------------------------------------------------------ the five BASELINE.json configs
