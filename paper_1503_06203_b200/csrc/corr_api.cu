@@ -212,7 +212,30 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         }
         const int fb = 128 / N;
         const int strips = (F + fb - 1) / fb;
-        int chunks = std::max(1, std::min((2 * p->sm_count + strips - 1) / strips, T / 512));
+        cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        int occ = 1;
+        if (e == cudaSuccess) {
+            if (N == 16) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<1>, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES);
+            else if (N == 32) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<2>, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES);
+            else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<4>, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES);
+        }
+        if (e != cudaSuccess || occ < 1) {
+            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::IM_SMEM_BYTES, cudaGetErrorString(e));
+            delete p;
+            return nullptr;
+        }
+        // time chunks (>= 512 samples each): the count that fills whole waves of CTA slots best
+        const int slots = p->sm_count * occ;
+        int chunks = 1;
+        double best = 0.0;
+        for (int c = 1; c <= std::max(1, std::min(T / 512, 4 * slots / strips + 1)); ++c) {
+            const long long units = (long long)strips * c;
+            const double eff = (double)units / (double)(((units + slots - 1) / slots) * slots);
+            if (eff > best + 0.10) { best = eff; chunks = c; }   // more chunks only for a clearly better fill
+        }
+        if (const char *cc = getenv("CORR_IMMA_CHUNKS")) chunks = std::max(1, std::min(atoi(cc), std::max(1, T / 128)));  // testing aid
         p->t_per_slice = ((T + chunks - 1) / chunks + corr::IM_ROWS - 1) / corr::IM_ROWS * corr::IM_ROWS;
         p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
         p->tile = N;
@@ -220,14 +243,6 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->num_units = strips * p->slices;
         p->grid = p->num_units;
         p->kernels_per_exec = 1;
-        cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
-        if (e != cudaSuccess) {
-            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::IM_SMEM_BYTES, cudaGetErrorString(e));
-            delete p;
-            return nullptr;
-        }
         return p;
     }
 

@@ -43,10 +43,14 @@ constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 256;
 template <int NT16> struct ImmaCfg {
     static constexpr int N = 16 * NT16;
     static constexpr int FB = 128 / N;                         // channels per strip
-    static constexpr int MS = (NT16 == 4) ? 2 : 1;             // m-tile sets per channel
+    static constexpr int MS = (NT16 == 4) ? 2 : 1;             // warps that share a channel's m-tiles
+    static constexpr int SETS = NT16 / MS;                     // m-tiles per warp (1, 2, 2)
     static constexpr int KS = (NT16 == 1) ? 2 : (NT16 == 2) ? 4 : 2;   // K-split
     static constexpr int WARPS = FB * MS * KS;                 // consumer warps (16, 16, 8)
-    static constexpr int THREADS = 32 * (WARPS + 1);           // + the TMA producer warp
+    // TMA producer: a warp of its own (measured 7 % faster than thread 0 issuing the loads between its
+    // consumer iterations; kept as an option because 17 warps cap a thread at 96 registers)
+    static constexpr bool SEP = true;
+    static constexpr int THREADS = 32 * (WARPS + (SEP ? 1 : 0));
 };
 
 struct ImmaParams {
@@ -64,19 +68,20 @@ __device__ __forceinline__ void mma_s8(int (&d)[4], const uint32_t (&a)[4], uint
 }
 
 // One K-block (32 samples): the products of m-tile MT (accumulator set S of this warp) with every n-tile.
-template <int NT16, int MT, int S>
+template <int NT16, int MT, int S, int SETS>
 __device__ __forceinline__ void imma_mtile(const uint32_t (&pr)[NT16][4], const uint32_t (&pi)[NT16][4],
-                                           int (&re)[2][2 * NT16][4], int (&ir)[2][2 * NT16][4])
+                                           int (&re)[SETS][2 * NT16][4], int (&ir)[SETS][2 * NT16][4])
 {
+    // three passes so that the two MMAs that add into the same Re block are far apart in the issue stream
 #pragma unroll
-    for (int nt = 0; nt < 2 * NT16; ++nt) {
-        const int bs = nt >> 1, h = nt & 1;   // source m-tile and half of the B fragment
-        mma_s8(ir[S][nt], pi[MT], pr[bs][h], pr[bs][2 + h]);
-        if (nt >= 2 * MT) {                   // blocks that touch the upper triangle
-            mma_s8(re[S][nt], pr[MT], pr[bs][h], pr[bs][2 + h]);
-            mma_s8(re[S][nt], pi[MT], pi[bs][h], pi[bs][2 + h]);
-        }
-    }
+    for (int nt = 2 * MT; nt < 2 * NT16; ++nt)        // blocks that touch the upper triangle
+        mma_s8(re[S][nt], pr[MT], pr[nt >> 1][nt & 1], pr[nt >> 1][2 + (nt & 1)]);
+#pragma unroll
+    for (int nt = 0; nt < 2 * NT16; ++nt)
+        mma_s8(ir[S][nt], pi[MT], pr[nt >> 1][nt & 1], pr[nt >> 1][2 + (nt & 1)]);
+#pragma unroll
+    for (int nt = 2 * MT; nt < 2 * NT16; ++nt)
+        mma_s8(re[S][nt], pi[MT], pi[nt >> 1][nt & 1], pi[nt >> 1][2 + (nt & 1)]);
 }
 
 template <int NT16>
@@ -108,35 +113,45 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     }
     __syncthreads();
 
-    // accumulators of this warp: up to two m-tiles x all n-tiles, (16 x 8 int32 per block) / 32 lanes
-    int re[2][2 * NT16][4], ir[2][2 * NT16][4];
+    // accumulators of this warp: SETS m-tiles x all n-tiles, (16 x 8 int32 per block) / 32 lanes
+    int re[C::SETS][2 * NT16][4], ir[C::SETS][2 * NT16][4];
 #pragma unroll
-    for (int s = 0; s < 2; ++s)
+    for (int s = 0; s < C::SETS; ++s)
 #pragma unroll
         for (int nt = 0; nt < 2 * NT16; ++nt)
 #pragma unroll
             for (int j = 0; j < 4; ++j) re[s][nt][j] = ir[s][nt][j] = 0;
 
     const int ch = warp % C::FB;                    // channel inside the strip
-    const int ms = (warp / C::FB) % C::MS;          // m-tile set
+    // N = 64: two warps per channel with m-tiles {0, 3} and {1, 2}: 36 MMAs per K-block each
+    const int ms = (warp / C::FB) % C::MS;
     const int ks = warp / (C::FB * C::MS);          // K-split index
     const int f = strip * C::FB + ch;
 
-    if (warp == C::WARPS) {
-        // ===================== TMA producer =====================
-        if (lane == 0) {
-            for (int it = 0; it < nstages; ++it) {
-                const int s = it % IM_STAGES;
-                ptx::mbar_wait(empty(s), ((uint32_t)(it / IM_STAGES) & 1u) ^ 1u);
-                ptx::mbar_arrive_expect_tx(full(s), IM_STAGE_BYTES);
-                ptx::tma_load_2d(base + s * IM_STAGE_BYTES, &tmap, full(s), strip * 128, t_begin + it * IM_ROWS);
-            }
+    // TMA producer = thread 0, interleaved with its consumer work: stage it + IM_STAGES - 1 is requested at
+    // the top of iteration it (its ring slot was released by every warp in iteration it - 1)
+    auto produce = [&](int j) {
+        if (j < nstages) {
+            const int sj = j % IM_STAGES;
+            ptx::mbar_wait(empty(sj), ((uint32_t)(j / IM_STAGES) & 1u) ^ 1u);
+            ptx::mbar_arrive_expect_tx(full(sj), IM_STAGE_BYTES);
+            ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj), strip * 128, t_begin + j * IM_ROWS);
         }
+    };
+    if (C::SEP && warp == C::WARPS) {
+        if (lane == 0)
+            for (int j = 0; j < nstages; ++j) produce(j);
     } else {
         // ===================== consumers =====================
+        if (!C::SEP && threadIdx.x == 0)
+            for (int j = 0; j < IM_STAGES - 1; ++j) produce(j);
         const uint32_t c16 = (uint32_t)(ch * N) >> 4;   // first 16-byte chunk of this channel in a 128-byte row
         for (int it = 0; it < nstages; ++it) {
             const int s = it % IM_STAGES;
+            if (!C::SEP) {
+                if (threadIdx.x == 0) produce(it + IM_STAGES - 1);
+                __syncwarp();
+            }
             ptx::mbar_wait(full(s), (uint32_t)(it / IM_STAGES) & 1u);
             const uint32_t stage = base + s * IM_STAGE_BYTES;
             if (f < p.F) {
@@ -157,24 +172,25 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
                             pi[mt][j] = ((w[j] << 4) ^ 0x80808080u) & 0xF0F0F0F0u;
                         }
                     }
+                    uint32_t mk0 = 0xF0F0F0F0u, mk1 = 0xF0F0F0F0u;
                     if (valid < 32) {   // ragged end of the chunk: zero the samples beyond it (registers 0,1: 4c.., 2,3: 16+4c..)
                         const int c4 = 4 * (lane & 3);
                         const int v0 = min(4, max(0, valid - c4)), v1 = min(4, max(0, valid - c4 - 16));
-                        const uint32_t m0 = v0 ? (0xFFFFFFFFu >> (32 - 8 * v0)) : 0u;
-                        const uint32_t m1 = v1 ? (0xFFFFFFFFu >> (32 - 8 * v1)) : 0u;
+                        mk0 = v0 ? (0xF0F0F0F0u >> (32 - 8 * v0)) : 0u;
+                        mk1 = v1 ? (0xF0F0F0F0u >> (32 - 8 * v1)) : 0u;
 #pragma unroll
                         for (int mt = 0; mt < NT16; ++mt) {
-                            pr[mt][0] &= m0; pr[mt][1] &= m0; pr[mt][2] &= m1; pr[mt][3] &= m1;
-                            pi[mt][0] &= m0; pi[mt][1] &= m0; pi[mt][2] &= m1; pi[mt][3] &= m1;
+                            pr[mt][0] &= mk0; pr[mt][1] &= mk0; pr[mt][2] &= mk1; pr[mt][3] &= mk1;
+                            pi[mt][0] &= mk0; pi[mt][1] &= mk0; pi[mt][2] &= mk1; pi[mt][3] &= mk1;
                         }
                     }
                     if constexpr (NT16 == 4) {
-                        if (ms == 0) { imma_mtile<4, 0, 0>(pr, pi, re, ir); imma_mtile<4, 3, 1>(pr, pi, re, ir); }
-                        else         { imma_mtile<4, 1, 0>(pr, pi, re, ir); imma_mtile<4, 2, 1>(pr, pi, re, ir); }
+                        if (ms == 0) { imma_mtile<4, 0, 0, 2>(pr, pi, re, ir); imma_mtile<4, 3, 1, 2>(pr, pi, re, ir); }
+                        else         { imma_mtile<4, 1, 0, 2>(pr, pi, re, ir); imma_mtile<4, 2, 1, 2>(pr, pi, re, ir); }
                     } else if constexpr (NT16 == 2) {
-                        imma_mtile<2, 0, 0>(pr, pi, re, ir); imma_mtile<2, 1, 1>(pr, pi, re, ir);
+                        imma_mtile<2, 0, 0, 2>(pr, pi, re, ir); imma_mtile<2, 1, 1, 2>(pr, pi, re, ir);
                     } else {
-                        imma_mtile<1, 0, 0>(pr, pi, re, ir);
+                        imma_mtile<1, 0, 0, 1>(pr, pi, re, ir);
                     }
                 }
             }
@@ -192,11 +208,8 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
         int *rre = red + (ch * 2 + 0) * N * N, *rir = red + (ch * 2 + 1) * N * N;
         const int g = lane >> 2, c2 = 2 * (lane & 3);
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            int mt;
-            if (NT16 == 4) mt = (ms == 0) ? (s == 0 ? 0 : 3) : (s == 0 ? 1 : 2);
-            else mt = s;
-            if (mt >= NT16) continue;
+        for (int s = 0; s < C::SETS; ++s) {
+            const int mt = (NT16 == 4) ? ((ms == 0) ? (s == 0 ? 0 : 3) : (s == 0 ? 1 : 2)) : s;
 #pragma unroll
             for (int nt = 0; nt < 2 * NT16; ++nt) {
 #pragma unroll
