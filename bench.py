@@ -234,15 +234,30 @@ def main():
     int8_peak = 2.0 * float(peaks["bf16_tflops"])  # dense int8 : bf16 nominal ratio is 2 (4.5 / 2.25 PF)
     kernel_ms = ms_per_step  # one kernel launch per step; launch gaps are inside the figure
     achieved = eff_ops(N, F, T) / (kernel_ms * 1e-3) / 1e12
-    roofline = {
-        "bound": "tensor", "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak,
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH if args.config == "cfg3" else None,
-        "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
-        "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
-        "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
-        "kernel": "corr_tc3_kernel", "kernel_ms": kernel_ms,
-        "algorithmic_ops_per_launch": eff_ops(N, F, T),
-    }
+    path = plan.info["path"]
+    if path == corr.PATH_TCGEN05:
+        variant = os.environ.get("CORR_TC_VARIANT", "3")
+        kernel = {"1": "corr_tc_kernel", "2": "corr_tc2_kernel", "4": "corr_tc4_kernel"}.get(variant, "corr_tc3_kernel")
+        roofline = {
+            "bound": "tensor", "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak,
+            "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == "cfg3" and kernel == "corr_tc3_kernel") else None,
+            "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
+            "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
+            "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
+            "kernel": kernel, "kernel_ms": kernel_ms,
+            "algorithmic_ops_per_launch": eff_ops(N, F, T),
+        }
+    else:
+        # small-N paths: one input byte per (sample, input) in, the (tiny) triangle out
+        alg_bytes = float(N * F * T + vis.numel() * 4)
+        gbs = alg_bytes / (kernel_ms * 1e-3) / 1e9
+        roofline = {
+            "bound": "hbm", "achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+            "frac": gbs / float(peaks["hbm_gbs"]), "traffic": None,
+            "peak_source": f"hbm_gbs of MEASURED_PEAKS.json ({peaks_kind})",
+            "kernel": "corr_imma_kernel" if path == corr.PATH_IMMA else "corr_dp4a_kernel", "kernel_ms": kernel_ms,
+            "algorithmic_bytes_per_launch": alg_bytes,
+        }
     cpu_baseline = None
     if not args.no_cpu_baseline:
         import oracle

@@ -69,8 +69,12 @@ enum {
  *   N  number of input elements,           N >= 1
  *   F  number of frequency channels,       F >= 1
  *   T  time samples per corr_execute call, 1 <= T <= 16 777 215
- * Returns NULL on failure; the reason is in corr_last_error().  The environment variable
- * CORR_FORCE_PATH=dp4a|tcgen05 overrides the automatic choice (testing aid). */
+ * Returns NULL on failure; the reason is in corr_last_error().
+ * Automatic choice: N = 16, 32, 64 -> CORR_PATH_IMMA; N % 16 == 0 and N >= 96 -> CORR_PATH_TCGEN05;
+ * everything else -> CORR_PATH_DP4A.  Testing aids (environment, read at plan creation):
+ * CORR_FORCE_PATH=dp4a|tcgen05|imma overrides the choice; CORR_TC_VARIANT=1|2|3|4 selects the
+ * tcgen05 kernel (default 3; 4 = three products per complex MAC with the Eq. 3 offset
+ * correction). */
 corr_plan *corr_plan_create(int N, int F, int T);
 
 /* Same, with the path given explicitly (CORR_PATH_*).  CORR_ERR_UNSUPPORTED -> NULL if the
