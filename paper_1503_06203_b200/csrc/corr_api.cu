@@ -91,6 +91,10 @@ struct corr_plan {
     int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128, operands in smem
                        // (corr_tc2.cuh); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
                        // 4: as 3 with three products per complex MAC (corr_tc4.cuh; CORR_TC_VARIANT=4)
+    int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
+    long long total_groups;
+    int *flags_dev;    // variant 3: [num_units][2] stream-K flags (corr_tc3.cuh)
+    int epoch;         // corr_execute calls so far
     int32_t *sums_dev; // variant 4: [2][slices][F][N] per-element sums of the stored bytes
     CUtensorMap tmap;
     CUtensorMap tmap_y;
@@ -138,6 +142,7 @@ void corr_plan_destroy(corr_plan *p)
     if (!p) return;
     if (p->tiles_dev) cudaFree(p->tiles_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
+    if (p->flags_dev) cudaFree(p->flags_dev);
     if (p->packed_own) cudaFree(p->packed_own);
     if (p->vis_own) cudaFree(p->vis_own);
     delete p;
@@ -288,7 +293,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     const int min_slices = (T + max_slice - 1) / max_slice;
     double best_cost = 0;
     int best_s = 0;
-    for (int s = min_slices; s <= std::max(min_slices, 64); ++s) {
+    // variant 3 balances the load itself (stream-K over groups of stages): T is split only for int32 headroom
+    const int s_max = (p->variant == 3) ? min_slices : std::max(min_slices, 64);
+    for (int s = min_slices; s <= s_max; ++s) {
         int tps = ((T + s - 1) / s + quantum - 1) / quantum * quantum;
         if (s > min_slices && tps < 8 * quantum) break;
         const int s_eff = (T + tps - 1) / tps;
@@ -307,6 +314,19 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
                                   : std::min(p->num_units, p->sm_count);
     p->kernels_per_exec = (p->variant == 4) ? 2 : 1;  // tc4: corr_sums_kernel + corr_tc4_kernel
     p->aligned = (N % 4 == 0) ? 1 : 0;
+    if (p->variant == 3) {
+        p->groups_full = p->t_per_slice / corr::T3_GROUP;
+        p->groups_last = (T - (p->slices - 1) * p->t_per_slice + corr::T3_GROUP - 1) / corr::T3_GROUP;
+        p->total_groups = units0 * ((long long)(p->slices - 1) * p->groups_full + p->groups_last);
+        p->grid = 2 * (int)std::min<long long>(p->total_groups, p->sm_count / 2);
+        if (cudaMalloc(&p->flags_dev, 2 * (size_t)p->num_units * sizeof(int)) != cudaSuccess ||
+            cudaMemset(p->flags_dev, 0, 2 * (size_t)p->num_units * sizeof(int)) != cudaSuccess) {
+            set_err("corr_plan_create: device allocation of the schedule flags failed: %s",
+                    cudaGetErrorString(cudaGetLastError()));
+            corr_plan_destroy(p);
+            return nullptr;
+        }
+    }
 
     if (cudaMalloc(&p->tiles_dev, tiles.size() * sizeof(ushort2)) != cudaSuccess ||
         cudaMemcpy(p->tiles_dev, tiles.data(), tiles.size() * sizeof(ushort2), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -476,6 +496,15 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.t_per_slice = p->t_per_slice;
             prm.num_units = p->num_units;
             prm.out_mode = out_mode;
+            prm.groups_full = p->groups_full;
+            prm.groups_last = p->groups_last;
+            prm.total_groups = p->total_groups;
+            if (p->epoch == 0x7fffffff) {   // the call counter wraps: forget every flag of the previous era
+                CUDA_TRY(cudaMemsetAsync(p->flags_dev, 0, 2 * (size_t)p->num_units * sizeof(int), stream), CORR_ERR_CUDA);
+                p->epoch = 0;
+            }
+            prm.epoch = ++p->epoch;
+            prm.flags = p->flags_dev;
             prm.tiles = p->tiles_dev;
             prm.vis = vis_dev;
             corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);

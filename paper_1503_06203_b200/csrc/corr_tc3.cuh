@@ -61,16 +61,89 @@ constexpr int T3_SMEM_BYTES = 1024 + T3_PK_STAGES * T3_PK_BYTES + T3_PL_STAGES *
 constexpr uint32_t T3_ACOL0 = 384;                 // first TMEM column of the A stages
 constexpr uint32_t T3_ACOLS = 32;                  // columns per A stage: Ar 16 | Ai 16
 
+constexpr int T3_GROUP = T3_ST * T3_PL_STAGES;   // samples per group of stages: the scheduling quantum
+
 struct Tc3Params {
     int N, F, T;
     int tiles_per_f;   // pair tiles (256 x 128) touching the upper triangle, per channel
     int slices;
-    int t_per_slice;   // multiple of T3_ST
+    int t_per_slice;   // multiple of T3_GROUP
     int num_units;     // F * tiles_per_f * slices
     int out_mode;
+    int groups_full;   // groups of T3_GROUP samples in a full slice
+    int groups_last;   // ... in the last slice of a tile
+    long long total_groups;  // over all units
+    int epoch;         // corr_execute call counter of the plan, > 0
+    int *flags;        // [num_units][2]: == epoch once the storing segment of (unit, CTA rank) is in memory
     const ushort2 *tiles;  // (bx2, by): x-block of 256, y-block of 128
     int32_t *vis;
 };
+
+// S3, second half: the work of a call is the list of units (channel, tile, T-slice), each a run of groups
+// of T3_GROUP samples.  Whole waves of units are dealt round-robin (unit = pair + k * npairs: the pairs then
+// work on neighbouring tiles of one channel at the same time, which is what keeps the re-read input in L2).
+// The units left over after the last whole wave are cut into one contiguous range of groups per CTA pair
+// ("stream-K"), so the tail costs every pair the same time whatever the number of tiles.  A segment is
+// the part of one unit that one pair computes: a whole unit, or a piece of a tail unit.
+struct Tc3Seg {
+    int u, f, slice;
+    ushort2 tile;
+    int first, cnt, len;   // groups [first, first + cnt) of the unit's len groups
+    int t_begin, t_end;    // first sample of the segment; end of the unit's slice (<= T)
+};
+
+struct Tc3Iter {
+    int k, waves, pair, npairs;
+    long long g, g_end;
+};
+
+__device__ __forceinline__ Tc3Iter tc3_iter(const Tc3Params &p, int pair, int npairs)
+{
+    Tc3Iter it;
+    it.k = 0;
+    it.waves = p.num_units / npairs;
+    it.pair = pair;
+    it.npairs = npairs;
+    // first group of the first tail unit in the linear order of units
+    const int u0 = it.waves * npairs;
+    const int full = (p.slices - 1) * p.groups_full;
+    const long long g0 = (long long)(u0 / p.slices) * (full + p.groups_last) + (long long)(u0 % p.slices) * p.groups_full;
+    const long long tail = p.total_groups - g0;
+    it.g = g0 + tail * pair / npairs;
+    it.g_end = g0 + tail * (pair + 1) / npairs;
+    return it;
+}
+
+__device__ __forceinline__ bool tc3_next_segment(const Tc3Params &p, Tc3Iter &it, Tc3Seg &s)
+{
+    const int full = (p.slices - 1) * p.groups_full;
+    const int per_ft = full + p.groups_last;
+    long long ft;
+    if (it.k < it.waves) {               // a whole unit of a whole wave
+        const int u = it.pair + it.k * it.npairs;
+        ++it.k;
+        ft = u / p.slices;
+        s.slice = u % p.slices;
+        s.first = 0;
+        s.len = (s.slice == p.slices - 1) ? p.groups_last : p.groups_full;
+        s.cnt = s.len;
+    } else {                             // this pair's share of the tail units
+        if (it.g >= it.g_end) return false;
+        ft = it.g / per_ft;
+        const int r = (int)(it.g - ft * per_ft);
+        s.slice = (r < full) ? r / p.groups_full : p.slices - 1;
+        s.first = r - s.slice * p.groups_full;
+        s.len = (s.slice == p.slices - 1) ? p.groups_last : p.groups_full;
+        s.cnt = (int)min((long long)(s.len - s.first), it.g_end - it.g);
+        it.g += s.cnt;
+    }
+    s.f = (int)(ft / p.tiles_per_f);
+    s.tile = p.tiles[(int)(ft % p.tiles_per_f)];
+    s.u = (int)ft * p.slices + s.slice;
+    s.t_begin = s.slice * p.t_per_slice + s.first * T3_GROUP;
+    s.t_end = min(p.T, (s.slice + 1) * p.t_per_slice);
+    return true;
+}
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
 corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ CUtensorMap tmap_y,
@@ -122,23 +195,21 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     const uint32_t tmem = *tmem_slot_g;
     if (tmem != 0) __trap();  // all 512 columns were requested: the allocation starts at lane 0, column 0
 
-    const int units_per_f = p.tiles_per_f * p.slices;
+    Tc3Iter sit = tc3_iter(p, pair, npairs);   // every role walks the same list of segments
+    Tc3Seg sg;
 
     if (warp == 0) {
         // ===================== S1: TMA producer (each CTA loads its own blocks) =====================
         if (lane == 0) {
             int st = 0;
             uint32_t ph = 0;
-            for (int u = pair; u < p.num_units; u += npairs) {
-                const int f = u / units_per_f, rem = u % units_per_f;
-                const ushort2 tile = p.tiles[rem / p.slices];
-                const int slice = rem % p.slices;
-                const int t_begin = slice * p.t_per_slice;
-                const int t_end = min(p.T, t_begin + p.t_per_slice);
+            while (tc3_next_segment(p, sit, sg)) {
+                const int f = sg.f;
+                const ushort2 tile = sg.tile;
+                const int t_begin = sg.t_begin;
                 const int xc = tile.x * 256 + (int)rank * 128;
                 const int yc = tile.y * 128 + (int)rank * 64;
-                const int t_pad = t_begin + (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES) *
-                                                (T3_ST * T3_PL_STAGES);  // every unit runs whole groups of stages
+                const int t_pad = t_begin + sg.cnt * T3_GROUP;   // whole groups of stages
                 for (int t = t_begin; t < t_pad; t += T3_ST) {
                     ptx::mbar_wait(pk_empty(st), ph ^ 1u);
                     ptx::mbar_arrive_expect_tx(pk_full(st), T3_PK_BYTES);
@@ -159,12 +230,8 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             constexpr uint32_t idesc = make_idesc_i8(256, 128, true, true, /*A K-major (TMEM)*/ false, /*B MN-major*/ true);
             uint32_t ph = 0, acc_ph = 0;
             const bool issuer = ptx::elect_one();
-            for (int u = pair; u < p.num_units; u += npairs) {
-                const int rem = u % units_per_f;
-                const int slice = rem % p.slices;
-                const int t_begin = slice * p.t_per_slice;
-                const int t_end = min(p.T, t_begin + p.t_per_slice);
-                const int ngroups = (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES);
+            while (tc3_next_segment(p, sit, sg)) {
+                const int ngroups = sg.cnt;
                 ptx::mbar_wait_cluster(acc_empty, acc_ph ^ 1u);
                 ptx::tc_fence_after_sync();
                 uint32_t acc = 0;
@@ -212,13 +279,9 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         const uint32_t tdst = tmem + ((uint32_t)(32 * q) << 16) + T3_ACOL0 + 8u * kh;
         int pst = 0, qst = 0;
         uint32_t pph = 0, qph = 0;
-        for (int u = pair; u < p.num_units; u += npairs) {
-            const int rem = u % units_per_f;
-            const int slice = rem % p.slices;
-            const int t_begin = slice * p.t_per_slice;
-            const int t_end = min(p.T, t_begin + p.t_per_slice);
-            const int t_pad = t_begin + (t_end - t_begin + T3_ST * T3_PL_STAGES - 1) / (T3_ST * T3_PL_STAGES) *
-                                            (T3_ST * T3_PL_STAGES);
+        while (tc3_next_segment(p, sit, sg)) {
+            const int t_begin = sg.t_begin, t_end = sg.t_end;
+            const int t_pad = t_begin + sg.cnt * T3_GROUP;
             for (int t = t_begin; t < t_pad; t += T3_ST) {
                 const int rows_valid = t_end - t;  // <= 0 in a padding stage: all-zero operands
                 // byte masks of this thread's four samples (zero beyond the slice)
@@ -289,11 +352,20 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         const uint32_t srow = epi0 + (uint32_t)row * T3_EPI_PITCH;
         uint8_t *srow_g = epi_g + row * T3_EPI_PITCH;
         const long long Bn = (long long)p.N * ((long long)p.N + 1) / 2;
-        const bool add = (p.out_mode != OUT_STORE);
+        const bool base_add = (p.out_mode != OUT_STORE);
         uint32_t acc_ph = 0;
-        for (int u = pair; u < p.num_units; u += npairs) {
-            const int f = u / units_per_f, rem = u % units_per_f;
-            const ushort2 tile = p.tiles[rem / p.slices];
+        while (tc3_next_segment(p, sit, sg)) {
+            // A unit cut by the stream-K schedule is summed in memory.  When the call overwrites (OUT_STORE),
+            // the segment that ends the unit stores and then raises the unit's flag; every other segment of
+            // the unit waits for the flag and adds.  The storing segment is always the FIRST work of its CTA
+            // pair (a pair's range is contiguous), so it never waits on anything: no deadlock.
+            const bool partial = (sg.cnt != sg.len), last = (sg.first + sg.cnt == sg.len);
+            const bool add = base_add || (partial && !last);
+            const bool wait_flag = !base_add && partial && !last;
+            const bool raise_flag = !base_add && partial && last;
+            int *flag = p.flags + 2 * sg.u + (int)rank;
+            const int f = sg.f;
+            const ushort2 tile = sg.tile;
             const int x0 = tile.x * 256 + (int)rank * 128, y0 = tile.y * 128;
             const int xw = x0 + q * 32;
             const int x = x0 + row;
@@ -332,6 +404,9 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
             // ---- write the row segment [jlo, jhi) of this thread
             int jlo = max(64 * h, x - y0), jhi = min(64 * h + 64, p.N - y0);
+            if (wait_flag)
+                while (ptx::ld_acquire_gpu(flag) != p.epoch) {
+                }
             if (x < p.N && jlo < jhi) {
                 ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
                 if ((par + jlo) & 1) {           // leading baseline on an odd 8-byte slot
@@ -352,6 +427,12 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                 }
             }
             ptx::bulk_commit();
+            if (raise_flag) {
+                ptx::bulk_wait0();                 // this thread's part of the tile is in memory ...
+                __threadfence();
+                ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);   // ... and so is every other epilogue thread's
+                if (threadIdx.x == 32 * T3_EPI_WARP0) ptx::st_release_gpu(flag, p.epoch);
+            }
         }
         ptx::bulk_wait0();  // every row segment has been written before the CTA retires
     }

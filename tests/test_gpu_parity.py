@@ -108,8 +108,12 @@ def test_tcgen05_extreme_values(corr, oracle):
 
 def test_split_t_and_multi_wave(corr, oracle):
     # few tiles, long T  -> the plan splits T (atomic accumulation); many tiles -> several waves
-    packed = workloads.iid_gaussian(256, 2, 20000, seed=77)
+    packed = workloads.iid_gaussian(256, 2, 20000, seed=77)   # 4 units on 74 CTA pairs: every unit is cut in many segments
     got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=123456)
+    assert info["units"] < info["ctas"] // 2
+    assert np.array_equal(got, oracle.level1(packed))
+    packed = workloads.iid_gaussian(256, 1, 40000, seed=79)   # T > 32768: sliced for int32 headroom as well
+    got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=-7)
     assert info["slices"] > 1
     assert np.array_equal(got, oracle.level1(packed))
     packed = workloads.iid_gaussian(1024, 8, 300, seed=78)
