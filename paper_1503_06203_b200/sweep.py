@@ -1,7 +1,7 @@
 """N sweep of the X-engine (the x-axis of the paper's Fig. 4) and the five BASELINE.json
 shapes: effective TOPS and achieved HBM GB/s per shape, device-timed with CUDA events.
 
-    python -m paper_1503_06203_b200.sweep [--reps 20] [--csv out.csv]
+    python -m paper_1503_06203_b200.sweep [--reps 20] [--csv out.csv] [--shape N,F,T]
 
 Inputs are random bytes generated on the device (every byte is a legal sample pair; timing does not
 depend on the values); correctness is the parity tests' job, not this script's.
@@ -26,14 +26,19 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--csv", default=None)
+    ap.add_argument("--shape", default=None, help="N,F,T: time this one shape only (e.g. under ncu)")
     args = ap.parse_args()
+    shapes = SHAPES
+    if args.shape:
+        n, f, t = (int(v) for v in args.shape.split(","))
+        shapes = [("shape", n, f, t, 0)]
     import torch
     from . import Plan
     if not torch.cuda.is_available():
         sys.exit("sweep needs a CUDA device (there is no CPU path)")
     dev = torch.device("cuda:0")
     rows = []
-    for label, N, F, T, acc in SHAPES:
+    for label, N, F, T, acc in shapes:
         plan = Plan(N, F, T)
         nbuf = 2 if N * F * T >= (64 << 20) else 8
         ins = [torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device=dev) for _ in range(nbuf)]
