@@ -98,7 +98,11 @@ int corr_execute(corr_plan *plan, const uint8_t *packed_dev, int32_t *vis_dev,
 /* corr_execute_host -- the same pass with HOST buffers: copies packed_host to a plan-owned
  * device buffer, runs corr_execute, copies the result back, all on `stream`, then synchronises
  * the stream.  With accumulate_flag != 0 vis_host is first copied to the device and added to.
- * Pinned host memory makes the copies asynchronous; pageable memory works but is slower. */
+ * Pinned host memory makes the copies asynchronous; pageable memory works but is slower.
+ * For large transfers (>= 32 MB, F > 1) the work is pipelined over groups of channels (channels
+ * are independent): the host->device copy of one group, the kernels of the previous
+ * one and the device->host copy of the one before run concurrently on plan-owned streams that
+ * are ordered after `stream` at entry and joined into it before the final synchronisation. */
 int corr_execute_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_host,
                       int accumulate_flag, corr_stream_t stream);
 

@@ -102,6 +102,11 @@ struct corr_plan {
     // corr_execute_host staging
     uint8_t *packed_own;
     int32_t *vis_own;
+    // corr_execute_host pipeline over groups of channels (copy in | compute | copy out)
+    corr_plan *sub;        // plan for host_fg channels, executed once per group
+    int host_fg;           // channels per group (divides F); 0 = not pipelined
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_start, ev_in[2], ev_free[2], ev_comp, ev_done;
 };
 
 extern "C" {
@@ -143,6 +148,18 @@ void corr_plan_destroy(corr_plan *p)
     if (p->tiles_dev) cudaFree(p->tiles_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->flags_dev) cudaFree(p->flags_dev);
+    if (p->sub) {
+        corr_plan_destroy(p->sub);
+        cudaStreamDestroy(p->s_in);
+        cudaStreamDestroy(p->s_out);
+        cudaEventDestroy(p->ev_start);
+        cudaEventDestroy(p->ev_comp);
+        cudaEventDestroy(p->ev_done);
+        for (int i = 0; i < 2; ++i) {
+            cudaEventDestroy(p->ev_in[i]);
+            cudaEventDestroy(p->ev_free[i]);
+        }
+    }
     if (p->packed_own) cudaFree(p->packed_own);
     if (p->vis_own) cudaFree(p->vis_own);
     delete p;
@@ -549,6 +566,71 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const size_t in_bytes = corr_input_bytes(p), out_bytes = corr_vis_elems(p) * sizeof(int32_t);
+
+    // Large transfers: pipeline over groups of channels (channels are independent), so that the
+    // host->device copy of group g+1, the kernels of group g and the device->host copy of group g-1 overlap
+    // (PCIe is full duplex).  Each group's slice of the stream is gathered by a strided 2-D copy into a
+    // contiguous [T][Fg][N] staging buffer (two of them, used alternately); its output is contiguous in vis.
+    if (p->host_fg == 0 && !p->sub) {
+        p->host_fg = -1;   // decided once
+        int groups = 0;
+        for (int g = std::min(p->F, 8); g >= 2; --g)
+            if (p->F % g == 0) { groups = g; break; }
+        if (groups >= 2 && in_bytes + out_bytes >= (size_t)(32 << 20)) {
+            corr_plan *sub = corr_plan_create_ex(p->N, p->F / groups, p->T, p->path);
+            if (sub) {
+                bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+                          cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess;
+                ok = ok && cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) == cudaSuccess &&
+                     cudaEventCreateWithFlags(&p->ev_comp, cudaEventDisableTiming) == cudaSuccess &&
+                     cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) == cudaSuccess;
+                for (int i = 0; i < 2 && ok; ++i)
+                    ok = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
+                         cudaEventCreateWithFlags(&p->ev_free[i], cudaEventDisableTiming) == cudaSuccess;
+                if (!ok) {
+                    set_err("corr_execute_host: cannot create the copy streams/events: %s", cudaGetErrorString(cudaGetLastError()));
+                    corr_plan_destroy(sub);
+                    return CORR_ERR_CUDA;
+                }
+                p->sub = sub;
+                p->host_fg = p->F / groups;
+            }
+        }
+    }
+    if (p->sub) {
+        const int fg = p->host_fg, groups = p->F / fg;
+        const size_t grp_in = (size_t)p->T * fg * p->N;
+        const size_t grp_out = (size_t)fg * ((size_t)p->N * (p->N + 1) / 2) * 2;   // int32 elements
+        if (!p->packed_own) CUDA_TRY(cudaMalloc(&p->packed_own, 2 * grp_in), CORR_ERR_ALLOC);
+        if (!p->vis_own) CUDA_TRY(cudaMalloc(&p->vis_own, out_bytes), CORR_ERR_ALLOC);
+        CUDA_TRY(cudaEventRecord(p->ev_start, stream), CORR_ERR_CUDA);       // everything follows the caller's stream
+        CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_start, 0), CORR_ERR_CUDA);
+        CUDA_TRY(cudaStreamWaitEvent(p->s_out, p->ev_start, 0), CORR_ERR_CUDA);
+        for (int g = 0; g < groups; ++g) {
+            const int b = g & 1;
+            uint8_t *din = p->packed_own + (size_t)b * grp_in;
+            int32_t *dvis = p->vis_own + (size_t)g * grp_out;
+            if (g >= 2) CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_free[b], 0), CORR_ERR_CUDA);   // staging buffer b is free again
+            CUDA_TRY(cudaMemcpy2DAsync(din, (size_t)fg * p->N, packed_host + (size_t)g * fg * p->N, (size_t)p->F * p->N,
+                                       (size_t)fg * p->N, (size_t)p->T, cudaMemcpyHostToDevice, p->s_in), CORR_ERR_CUDA);
+            if (accumulate_flag)
+                CUDA_TRY(cudaMemcpyAsync(dvis, vis_host + (size_t)g * grp_out, grp_out * sizeof(int32_t),
+                                         cudaMemcpyHostToDevice, p->s_in), CORR_ERR_CUDA);
+            CUDA_TRY(cudaEventRecord(p->ev_in[b], p->s_in), CORR_ERR_CUDA);
+            CUDA_TRY(cudaStreamWaitEvent(stream, p->ev_in[b], 0), CORR_ERR_CUDA);
+            int rc = corr_execute(p->sub, din, dvis, accumulate_flag, stream_);
+            if (rc != CORR_OK) return rc;
+            CUDA_TRY(cudaEventRecord(p->ev_free[b], stream), CORR_ERR_CUDA);
+            CUDA_TRY(cudaEventRecord(p->ev_comp, stream), CORR_ERR_CUDA);
+            CUDA_TRY(cudaStreamWaitEvent(p->s_out, p->ev_comp, 0), CORR_ERR_CUDA);
+            CUDA_TRY(cudaMemcpyAsync(vis_host + (size_t)g * grp_out, dvis, grp_out * sizeof(int32_t),
+                                     cudaMemcpyDeviceToHost, p->s_out), CORR_ERR_CUDA);
+        }
+        CUDA_TRY(cudaEventRecord(p->ev_done, p->s_out), CORR_ERR_CUDA);
+        CUDA_TRY(cudaStreamWaitEvent(stream, p->ev_done, 0), CORR_ERR_CUDA);
+        CUDA_TRY(cudaStreamSynchronize(stream), CORR_ERR_CUDA);
+        return CORR_OK;
+    }
     if (!p->packed_own) CUDA_TRY(cudaMalloc(&p->packed_own, in_bytes), CORR_ERR_ALLOC);
     if (!p->vis_own) CUDA_TRY(cudaMalloc(&p->vis_own, out_bytes), CORR_ERR_ALLOC);
     CUDA_TRY(cudaMemcpyAsync(p->packed_own, packed_host, in_bytes, cudaMemcpyHostToDevice, stream), CORR_ERR_CUDA);

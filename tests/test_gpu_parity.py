@@ -185,6 +185,24 @@ def test_execute_host(corr, oracle):
         assert np.array_equal(vh.numpy(), 2 * want)
 
 
+def test_execute_host_pipelined(corr, oracle):
+    # >= 32 MB of transfers and F > 1: corr_execute_host pipelines copy-in | kernels | copy-out over channel groups
+    import torch
+    packed = workloads.iid_gaussian(1024, 6, 5500, seed=21)
+    T, F, N = packed.shape
+    want = oracle.level1(packed)
+    with corr.Plan(N, F, T) as plan:
+        ph = torch.from_numpy(packed).pin_memory()
+        vh = torch.full((F, plan.baselines, 2), -559038737, dtype=torch.int32).pin_memory()
+        plan.execute_host(ph, vh, accumulate=False)
+        assert np.array_equal(vh.numpy(), want)
+        plan.execute_host(ph, vh, accumulate=True)
+        assert np.array_equal(vh.numpy(), 2 * want)
+        pageable = np.empty_like(want)                     # pageable host memory works too (just slower)
+        plan.execute_host(packed, pageable, accumulate=False)
+        assert np.array_equal(pageable, want)
+
+
 def test_invalid_arguments(corr):
     for bad in [(0, 1, 1), (16, 0, 1), (16, 1, 0), (16, 1, 1 << 24)]:
         with pytest.raises(corr.CorrError):
