@@ -203,6 +203,25 @@ def test_execute_host_pipelined(corr, oracle):
         assert np.array_equal(pageable, want)
 
 
+def test_int32_headroom_edge(corr):
+    # pin P10: the largest T the ABI takes, every sample -8-8i: Re = 128 * (2^24 - 1) =
+    # 2 147 483 520 on every baseline, Im = 0, no wrap (closed form, PAPER.md:41-44 with constant input)
+    import torch
+    N, F, T = 16, 1, (1 << 24) - 1
+    with corr.Plan(N, F, T) as plan:
+        dev = torch.zeros((T, F, N), dtype=torch.uint8, device="cuda")
+        vis = plan.execute(dev)
+        torch.cuda.synchronize()
+        got = vis.cpu().numpy()
+    assert (got[..., 0] == 2147483520).all() and (got[..., 1] == 0).all()
+    # the same length through the tcgen05 path (sliced for accumulator headroom), fewer samples to keep it short
+    N, T = 128, 100000
+    packed = np.zeros((T, 1, N), np.uint8)
+    got, info = _run(corr, packed, corr.PATH_TCGEN05)
+    assert info["slices"] > 1
+    assert (got[..., 0] == 128 * T).all() and (got[..., 1] == 0).all()
+
+
 def test_invalid_arguments(corr):
     for bad in [(0, 1, 1), (16, 0, 1), (16, 1, 0), (16, 1, 1 << 24)]:
         with pytest.raises(corr.CorrError):
