@@ -106,6 +106,19 @@ int corr_execute(corr_plan *plan, const uint8_t *packed_dev, int32_t *vis_dev,
 int corr_execute_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_host,
                       int accumulate_flag, corr_stream_t stream);
 
+/* corr_time_shift -- the paper's pre-correlation time shift ("modifies the input stream
+ * at the raw data level, allowing individual elements to be shifted by integer time steps
+ * pre-correlation"):
+ *     out[t][f][n] = in[t - lags[n]][f][n]  if 0 <= t - lags[n] < T,  else 0x88 (the sample 0 + 0i)
+ * A positive lag delays element n; samples shifted in from outside the block are stored zeros, which
+ * add nothing to any correlation sum.  Not in place.
+ *   packed_in_dev, packed_out_dev  DEVICE pointers, T*F*N bytes each, layout [T][F][N] as above,
+ *                                  distinct, 16-byte aligned when N % 16 == 0; caller-owned
+ *   lags_dev                       DEVICE pointer, N int32 (any values; |lag| >= T empties the element)
+ * Enqueues on `stream`, does not synchronise.  Returns CORR_OK or an error code. */
+int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int32_t *lags_dev,
+                    uint8_t *packed_out_dev, corr_stream_t stream);
+
 /* corr_plan_destroy -- free the plan and its device scratch.  NULL is a no-op. */
 void corr_plan_destroy(corr_plan *plan);
 

@@ -10,6 +10,7 @@ only compiles it and marshals numpy arrays.
     pair(packed, f, x, y)                  one ordered pair, any order (Hermitian pin)
     eq3_route(packed)                      stored-nibble products + Eq. 3 offsets
     baseline_index(N, x, y)                b(x,y) = x*N - x(x-1)/2 + (y-x)
+    time_shift(packed, lags)               per-element integer time shift, PAPER.md:125-131 (numpy)
 """
 from __future__ import annotations
 
@@ -131,3 +132,24 @@ def baseline_index(N: int, x: int, y: int) -> int:
 def threads() -> int:
     """OpenMP threads level1 will use (bench.py reports this as cpu_baseline.cores)."""
     return int(_load().corr_oracle_threads())
+
+
+def time_shift(packed: np.ndarray, lags) -> np.ndarray:
+    """The paper's pre-correlation time shift, written out as its definition:
+    out[t][f][n] = packed[t - lags[n]][f][n] if 0 <= t - lags[n] < T else 0x88 (the stored form of 0 + 0i).
+    Plain numpy, one input element at a time."""
+    packed = np.ascontiguousarray(packed, dtype=np.uint8)
+    T, F, N = packed.shape
+    lags = np.asarray(lags, dtype=np.int64)
+    if lags.shape != (N,):
+        raise ValueError("lags must have N entries")
+    out = np.full_like(packed, 0x88)
+    for n in range(N):
+        d = int(lags[n])
+        if d >= T or d <= -T:
+            continue
+        if d >= 0:
+            out[d:, :, n] = packed[:T - d, :, n]
+        else:
+            out[:T + d, :, n] = packed[-d:, :, n]
+    return out

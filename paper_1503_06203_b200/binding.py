@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift")
 
 
 class CorrError(RuntimeError):
@@ -57,6 +57,8 @@ def load_library():
         lib.corr_plan_info.restype = ci
         lib.corr_count_tiles.argtypes = [ci, ci, ci]
         lib.corr_count_tiles.restype = ci
+        lib.corr_time_shift.argtypes = [ci, ci, ci, vp, vp, vp, vp]
+        lib.corr_time_shift.restype = ci
         _lib = lib
     return _lib
 
@@ -84,6 +86,28 @@ def corr_execute_host(plan: int, packed_host_ptr: int, vis_host_ptr: int, accumu
     rc = load_library().corr_execute_host(plan, packed_host_ptr, vis_host_ptr, int(bool(accumulate_flag)), stream)
     if rc != 0:
         raise CorrError(f"corr_execute_host -> {rc}: {_err()}")
+
+
+def corr_time_shift(N: int, F: int, T: int, packed_in_ptr: int, lags_ptr: int, packed_out_ptr: int, stream: int) -> None:
+    rc = load_library().corr_time_shift(N, F, T, packed_in_ptr, lags_ptr, packed_out_ptr, stream)
+    if rc != 0:
+        raise CorrError(f"corr_time_shift -> {rc}: {_err()}")
+
+
+def time_shift(packed, lags, out=None, stream=None):
+    """packed: uint8 CUDA tensor [T][F][N]; lags: int32 CUDA tensor [N].  Returns the shifted stream
+    (a new tensor unless `out` is given).  Enqueues only."""
+    import torch
+    if not packed.is_cuda or packed.dtype != torch.uint8 or not packed.is_contiguous() or packed.dim() != 3:
+        raise ValueError("packed must be a contiguous uint8 CUDA tensor [T][F][N]")
+    T, F, N = packed.shape
+    if not lags.is_cuda or lags.dtype != torch.int32 or lags.numel() != N or not lags.is_contiguous():
+        raise ValueError("lags must be a contiguous int32 CUDA tensor of N elements")
+    if out is None:
+        out = torch.empty_like(packed)
+    s = torch.cuda.current_stream(packed.device) if stream is None else stream
+    corr_time_shift(N, F, T, packed.data_ptr(), lags.data_ptr(), out.data_ptr(), s.cuda_stream)
+    return out
 
 
 def corr_plan_destroy(plan: int) -> None:

@@ -14,6 +14,7 @@
 #include "../../include/corr.h"
 #include "corr_dp4a.cuh"
 #include "corr_imma.cuh"
+#include "corr_shift.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
 #include "corr_tc3.cuh"
@@ -380,6 +381,34 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
 }
 
 corr_plan *corr_plan_create(int N, int F, int T) { return corr_plan_create_ex(N, F, T, CORR_PATH_AUTO); }
+
+int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int32_t *lags_dev, uint8_t *packed_out_dev,
+                    corr_stream_t stream_)
+{
+    if (N < 1 || F < 1 || T < 1 || F > 65535 || (T + corr::SH_TB - 1) / corr::SH_TB > 65535) {
+        set_err("corr_time_shift: need N >= 1, 1 <= F <= 65535, 1 <= T <= %d (got N=%d F=%d T=%d)", 65535 * corr::SH_TB, N, F, T);
+        return CORR_ERR_INVALID_ARG;
+    }
+    if (!packed_in_dev || !lags_dev || !packed_out_dev || packed_in_dev == packed_out_dev) {
+        set_err("corr_time_shift: NULL buffer, or input and output are the same buffer (the shift is not in place)");
+        return CORR_ERR_INVALID_ARG;
+    }
+    if ((N % 16 == 0) && ((reinterpret_cast<uintptr_t>(packed_in_dev) | reinterpret_cast<uintptr_t>(packed_out_dev)) & 15u)) {
+        set_err("corr_time_shift: buffers must be 16-byte aligned");
+        return CORR_ERR_INVALID_ARG;
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(corr::corr_shift_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::SH_SMEM_BYTES),
+                 CORR_ERR_CUDA);
+        attr_set = true;
+    }
+    dim3 grid((unsigned)((N + 127) / 128), (unsigned)F, (unsigned)((T + corr::SH_TB - 1) / corr::SH_TB));
+    corr::corr_shift_kernel<<<grid, corr::SH_THREADS, corr::SH_SMEM_BYTES, static_cast<cudaStream_t>(stream_)>>>(
+        packed_in_dev, packed_out_dev, lags_dev, N, F, T);
+    CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+    return CORR_OK;
+}
 
 static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
 {
