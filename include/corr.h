@@ -106,6 +106,22 @@ int corr_execute(corr_plan *plan, const uint8_t *packed_dev, int32_t *vis_dev,
 int corr_execute_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_host,
                       int accumulate_flag, corr_stream_t stream);
 
+/* corr_execute_gated -- gated correlation ("gate the correlation products on multiple time
+ * periods", for periodic signals such as calibration sources and pulsars): every time sample t of the
+ * call belongs to gate gate[t] in [0, G), or to none (-1), and gate g gets its own matrix
+ *     vis[g][f][b(x,y)] (=|+=) sum over { t : gate[t] = g } of X_t[x] conj(X_t[y])
+ *   plan        a plan for (N, F, T); T is the length of gate[] and of the stream
+ *   packed_dev  DEVICE pointer, [T][F][N] bytes as for corr_execute
+ *   gate_host   HOST pointer, T int32; read before the call returns
+ *   G           number of gates, >= 1 (at most T distinct run lengths are planned and cached)
+ *   vis_dev     DEVICE pointer, G*F*N(N+1)/2*2 int32, layout [G][F][B][2]
+ *   accumulate_flag  as for corr_execute, applied to every gate (a gate with no sample is zeroed / left)
+ * Enqueues on `stream` (a row gather into plan-owned scratch, then one ordinary pass per gate); may
+ * wait for the previous gated call's index upload; the first call with a new run length creates a
+ * plan for it.  Returns CORR_OK or an error code. */
+int corr_execute_gated(corr_plan *plan, const uint8_t *packed_dev, const int32_t *gate_host, int G,
+                       int32_t *vis_dev, int accumulate_flag, corr_stream_t stream);
+
 /* corr_time_shift -- the paper's pre-correlation time shift ("modifies the input stream
  * at the raw data level, allowing individual elements to be shifted by integer time steps
  * pre-correlation"):

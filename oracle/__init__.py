@@ -11,6 +11,7 @@ only compiles it and marshals numpy arrays.
     eq3_route(packed)                      stored-nibble products + Eq. 3 offsets
     baseline_index(N, x, y)                b(x,y) = x*N - x(x-1)/2 + (y-x)
     time_shift(packed, lags)               per-element integer time shift, PAPER.md:125-131 (numpy)
+    gated(packed, gate, G)                 one matrix per gate of time samples
 """
 from __future__ import annotations
 
@@ -152,4 +153,21 @@ def time_shift(packed: np.ndarray, lags) -> np.ndarray:
             out[d:, :, n] = packed[:T - d, :, n]
         else:
             out[:T + d, :, n] = packed[-d:, :, n]
+    return out
+
+
+def gated(packed: np.ndarray, gate, G: int) -> np.ndarray:
+    """Gated correlation: vis[g] = Eq. 1 summed over the samples t with gate[t] == g
+    (gate -1 = in no gate).  The definition written out: select the samples of a gate, then the same
+    level-1 loops; a gate without samples is all zero.  Returns int32 [G][F][B][2]."""
+    packed = np.ascontiguousarray(packed, dtype=np.uint8)
+    T, F, N = packed.shape
+    gate = np.asarray(gate)
+    if gate.shape != (T,) or gate.min(initial=0) < -1 or gate.max(initial=-1) >= G:
+        raise ValueError("gate must have T entries in [-1, G)")
+    out = np.zeros((G, F, N * (N + 1) // 2, 2), np.int32)
+    for g in range(G):
+        sel = packed[gate == g]
+        if sel.shape[0]:
+            out[g] = level1(np.ascontiguousarray(sel))
     return out

@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated")
 
 
 class CorrError(RuntimeError):
@@ -57,6 +57,8 @@ def load_library():
         lib.corr_plan_info.restype = ci
         lib.corr_count_tiles.argtypes = [ci, ci, ci]
         lib.corr_count_tiles.restype = ci
+        lib.corr_execute_gated.argtypes = [vp, vp, vp, ci, vp, ci, vp]
+        lib.corr_execute_gated.restype = ci
         lib.corr_time_shift.argtypes = [ci, ci, ci, vp, vp, vp, vp]
         lib.corr_time_shift.restype = ci
         _lib = lib
@@ -86,6 +88,14 @@ def corr_execute_host(plan: int, packed_host_ptr: int, vis_host_ptr: int, accumu
     rc = load_library().corr_execute_host(plan, packed_host_ptr, vis_host_ptr, int(bool(accumulate_flag)), stream)
     if rc != 0:
         raise CorrError(f"corr_execute_host -> {rc}: {_err()}")
+
+
+def corr_execute_gated(plan: int, packed_dev_ptr: int, gate_host_ptr: int, G: int, vis_dev_ptr: int,
+                       accumulate_flag: int, stream: int) -> None:
+    rc = load_library().corr_execute_gated(plan, packed_dev_ptr, gate_host_ptr, G, vis_dev_ptr,
+                                           int(bool(accumulate_flag)), stream)
+    if rc != 0:
+        raise CorrError(f"corr_execute_gated -> {rc}: {_err()}")
 
 
 def corr_time_shift(N: int, F: int, T: int, packed_in_ptr: int, lags_ptr: int, packed_out_ptr: int, stream: int) -> None:
@@ -165,6 +175,26 @@ class Plan:
             raise ValueError("vis must be a contiguous int32 CUDA tensor of F*B*2 elements")
         s = torch.cuda.current_stream(packed.device) if stream is None else stream
         corr_execute(self._h, packed.data_ptr(), vis.data_ptr(), int(accumulate), s.cuda_stream)
+        return vis
+
+    def execute_gated(self, packed, gate, G: int, vis=None, accumulate: bool = False, stream=None):
+        """packed: uint8 CUDA tensor [T][F][N]; gate: T integers in [-1, G) (numpy array or list, host);
+        vis: int32 CUDA tensor [G][F][B][2] (allocated if None).  Enqueues; does not synchronise."""
+        import numpy as np
+        import torch
+        if not packed.is_cuda or packed.dtype != torch.uint8 or not packed.is_contiguous() or packed.numel() != self.input_bytes:
+            raise ValueError("packed must be a contiguous uint8 CUDA tensor of T*F*N bytes")
+        gate = np.ascontiguousarray(gate, dtype=np.int32)
+        if gate.shape != (self.T,):
+            raise ValueError("gate must have T entries")
+        if vis is None:
+            if accumulate:
+                raise ValueError("accumulate=True needs an existing vis tensor")
+            vis = torch.empty((G, self.F, self.baselines, 2), dtype=torch.int32, device=packed.device)
+        if not vis.is_cuda or vis.dtype != torch.int32 or not vis.is_contiguous() or vis.numel() != G * self.vis_elems:
+            raise ValueError("vis must be a contiguous int32 CUDA tensor of G*F*B*2 elements")
+        s = torch.cuda.current_stream(packed.device) if stream is None else stream
+        corr_execute_gated(self._h, packed.data_ptr(), gate.ctypes.data, G, vis.data_ptr(), int(accumulate), s.cuda_stream)
         return vis
 
     def execute_host(self, packed_host, vis_host, accumulate: bool = False, stream=None):

@@ -9,10 +9,12 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <vector>
 
 #include "../../include/corr.h"
 #include "corr_dp4a.cuh"
+#include "corr_gate.cuh"
 #include "corr_imma.cuh"
 #include "corr_shift.cuh"
 #include "corr_tc.cuh"
@@ -108,6 +110,12 @@ struct corr_plan {
     int host_fg;           // channels per group (divides F); 0 = not pipelined
     cudaStream_t s_in, s_out;
     cudaEvent_t ev_start, ev_in[2], ev_free[2], ev_comp, ev_done;
+    // corr_execute_gated: per-gate runs of the gathered stream, plans for their lengths
+    uint8_t *gate_buf;     // device, T*F*N bytes: rows regrouped by gate
+    int *order_dev;        // device, T row indices
+    int *order_pin;        // pinned host copy the upload reads from
+    cudaEvent_t ev_gate;   // the upload of order_pin has been consumed
+    std::map<int, corr_plan *> *gate_plans;   // length of a run -> plan (N, F, length)
 };
 
 extern "C" {
@@ -149,6 +157,16 @@ void corr_plan_destroy(corr_plan *p)
     if (p->tiles_dev) cudaFree(p->tiles_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->flags_dev) cudaFree(p->flags_dev);
+    if (p->gate_plans) {
+        for (auto &kv : *p->gate_plans) corr_plan_destroy(kv.second);
+        delete p->gate_plans;
+    }
+    if (p->gate_buf) cudaFree(p->gate_buf);
+    if (p->order_dev) cudaFree(p->order_dev);
+    if (p->order_pin) {
+        cudaFreeHost(p->order_pin);
+        cudaEventDestroy(p->ev_gate);
+    }
     if (p->sub) {
         corr_plan_destroy(p->sub);
         cudaStreamDestroy(p->s_in);
@@ -583,6 +601,95 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         }
     }
     CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+    return CORR_OK;
+}
+
+int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *gate_host, int G, int32_t *vis_dev,
+                       int accumulate_flag, corr_stream_t stream_)
+{
+    if (!p || !packed_dev || !gate_host || !vis_dev || G < 1) {
+        set_err("corr_execute_gated: NULL plan or buffer, or G < 1");
+        return CORR_ERR_INVALID_ARG;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const int T = p->T;
+    const size_t row_bytes = (size_t)p->F * p->N;
+    const size_t vis_per_gate = corr_vis_elems(p);
+    // ---- host: rows grouped by gate (stable), run lengths
+    std::vector<int> count((size_t)G, 0);
+    for (int t = 0; t < T; ++t) {
+        const int g = gate_host[t];
+        if (g >= G || g < -1) {
+            set_err("corr_execute_gated: gate[%d] = %d is outside [-1, %d)", t, g, G);
+            return CORR_ERR_INVALID_ARG;
+        }
+        if (g >= 0) ++count[(size_t)g];
+    }
+    if (!p->order_pin) {
+        CUDA_TRY(cudaMallocHost(&p->order_pin, (size_t)T * sizeof(int)), CORR_ERR_ALLOC);
+        CUDA_TRY(cudaEventCreateWithFlags(&p->ev_gate, cudaEventDisableTiming), CORR_ERR_CUDA);
+        CUDA_TRY(cudaMalloc(&p->order_dev, (size_t)T * sizeof(int)), CORR_ERR_ALLOC);
+        CUDA_TRY(cudaMalloc(&p->gate_buf, (size_t)T * row_bytes + 16 * (size_t)T + 16), CORR_ERR_ALLOC);   // + alignment padding per run
+        p->gate_plans = new std::map<int, corr_plan *>();
+    } else {
+        CUDA_TRY(cudaEventSynchronize(p->ev_gate), CORR_ERR_CUDA);   // the previous call's upload has left order_pin
+    }
+    std::vector<int> start((size_t)G + 1, 0);
+    for (int g = 0; g < G; ++g) start[(size_t)g + 1] = start[(size_t)g] + count[(size_t)g];
+    {
+        std::vector<int> fill(start.begin(), start.end() - 1);
+        for (int t = 0; t < T; ++t)
+            if (gate_host[t] >= 0) p->order_pin[fill[(size_t)gate_host[t]]++] = t;
+    }
+    const int used = start[(size_t)G];
+    // byte offset of every gate's run in gate_buf: runs start on 16-byte boundaries (corr_execute needs that)
+    std::vector<size_t> off((size_t)G, 0);
+    {
+        size_t o = 0;
+        for (int g = 0; g < G; ++g) {
+            off[(size_t)g] = o;
+            o = (o + (size_t)count[(size_t)g] * row_bytes + 15) & ~(size_t)15;
+        }
+    }
+    if (used > 0) {
+        CUDA_TRY(cudaMemcpyAsync(p->order_dev, p->order_pin, (size_t)used * sizeof(int), cudaMemcpyHostToDevice, stream),
+                 CORR_ERR_CUDA);
+        CUDA_TRY(cudaEventRecord(p->ev_gate, stream), CORR_ERR_CUDA);
+        const int blocks = 8 * p->sm_count;
+        if (row_bytes % 16 == 0) {   // runs are back to back: one launch for all gates
+            corr::corr_gate_gather_kernel<<<blocks, corr::GATE_THREADS, 0, stream>>>(packed_dev, p->gate_buf, p->order_dev, used,
+                                                                                     (int)(row_bytes / 16));
+        } else {
+            for (int g = 0; g < G; ++g)
+                if (count[(size_t)g] > 0)
+                    corr::corr_gate_gather_bytes_kernel<<<blocks, corr::GATE_THREADS, 0, stream>>>(
+                        packed_dev, p->gate_buf + off[(size_t)g], p->order_dev + start[(size_t)g], count[(size_t)g], (int)row_bytes);
+        }
+        CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+    } else {
+        CUDA_TRY(cudaEventRecord(p->ev_gate, stream), CORR_ERR_CUDA);
+    }
+    // ---- one ordinary correlation per gate on its run of rows
+    for (int g = 0; g < G; ++g) {
+        int32_t *vis_g = vis_dev + (size_t)g * vis_per_gate;
+        const int len = count[(size_t)g];
+        if (len == 0) {
+            if (!accumulate_flag) CUDA_TRY(cudaMemsetAsync(vis_g, 0, vis_per_gate * sizeof(int32_t), stream), CORR_ERR_CUDA);
+            continue;
+        }
+        auto it = p->gate_plans->find(len);
+        if (it == p->gate_plans->end()) {
+            if (p->gate_plans->size() >= 64) {   // bound the cache (cudaFree in destroy waits for the device)
+                for (auto &kv : *p->gate_plans) corr_plan_destroy(kv.second);
+                p->gate_plans->clear();
+            }
+            corr_plan *np = corr_plan_create_ex(p->N, p->F, len, p->path);
+            if (!np) return CORR_ERR_ALLOC;
+            it = p->gate_plans->emplace(len, np).first;
+        }
+        int rc = corr_execute(it->second, p->gate_buf + off[(size_t)g], vis_g, accumulate_flag, stream_);
+        if (rc != CORR_OK) return rc;
+    }
     return CORR_OK;
 }
 
