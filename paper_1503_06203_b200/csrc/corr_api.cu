@@ -88,6 +88,7 @@ struct corr_plan {
     int grid;
     int kernels_per_exec;
     ushort2 *tiles_dev;
+    ushort4 *tiles4_dev;   // variant 3: (xa, xb, by, flags), see Tc3Tile in corr_tc3.cuh
     // dp4a only
     int aligned;
     // tcgen05 only
@@ -155,6 +156,7 @@ void corr_plan_destroy(corr_plan *p)
 {
     if (!p) return;
     if (p->tiles_dev) cudaFree(p->tiles_dev);
+    if (p->tiles4_dev) cudaFree(p->tiles4_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->flags_dev) cudaFree(p->flags_dev);
     if (p->gate_plans) {
@@ -299,7 +301,24 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
-    if (p->variant >= 2) {
+    std::vector<ushort4> tiles4;
+    if (p->variant == 3) {
+        // Pair tiles of two row blocks (128 inputs each) against one column block.  Column block j needs the row
+        // blocks 0..j.  An even count pairs up as (0,1), (2,3), ...; an odd count as (1,2), (3,4), ... and leaves
+        // block (0, j) over.  The left-over blocks all have row block 0: computed transposed (rows = block j,
+        // columns = block 0) they share their column operand, so they pair up with each other.
+        auto us = [](int v) { return (unsigned short)v; };
+        std::vector<int> left;
+        for (int j = 0; j < nb; ++j) {
+            const int first = ((j + 1) % 2 == 0) ? 0 : 1;
+            for (int a = first; a + 1 <= j; a += 2) tiles4.push_back(make_ushort4(us(a), us(a + 1), us(j), 0));
+            if (first == 1) left.push_back(j);
+        }
+        for (size_t i = 0; i < left.size(); i += 2)
+            tiles4.push_back(make_ushort4(us(left[i]), (i + 1 < left.size()) ? us(left[i + 1]) : corr::TC3_NO_BLOCK, 0,
+                                          corr::TC3_TILE_TRANSPOSED));
+        tiles.resize(tiles4.size());   // the count is what the schedule below needs
+    } else if (p->variant >= 2) {
         // pair tiles: x-block of 256 (two CTAs x 128), y-block of 128; keep those whose largest y
         // reaches their smallest x
         const int nbx = (N + 255) / 256;
@@ -365,7 +384,10 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     }
 
     if (cudaMalloc(&p->tiles_dev, tiles.size() * sizeof(ushort2)) != cudaSuccess ||
-        cudaMemcpy(p->tiles_dev, tiles.data(), tiles.size() * sizeof(ushort2), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaMemcpy(p->tiles_dev, tiles.data(), tiles.size() * sizeof(ushort2), cudaMemcpyHostToDevice) != cudaSuccess ||
+        (!tiles4.empty() &&
+         (cudaMalloc(&p->tiles4_dev, tiles4.size() * sizeof(ushort4)) != cudaSuccess ||
+          cudaMemcpy(p->tiles4_dev, tiles4.data(), tiles4.size() * sizeof(ushort4), cudaMemcpyHostToDevice) != cudaSuccess))) {
         set_err("corr_plan_create: device allocation of the tile table failed: %s",
                 cudaGetErrorString(cudaGetLastError()));
         corr_plan_destroy(p);
@@ -569,7 +591,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             }
             prm.epoch = ++p->epoch;
             prm.flags = p->flags_dev;
-            prm.tiles = p->tiles_dev;
+            prm.tiles = p->tiles4_dev;
             prm.vis = vis_dev;
             corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
         } else if (p->variant == 2) {

@@ -75,7 +75,7 @@ struct Tc3Params {
     long long total_groups;  // over all units
     int epoch;         // corr_execute call counter of the plan, > 0
     int *flags;        // [num_units][2]: == epoch once the storing segment of (unit, CTA rank) is in memory
-    const ushort2 *tiles;  // (bx2, by): x-block of 256, y-block of 128
+    const ushort4 *tiles;  // (xa, xb, by, flags): 128-blocks of the rows of CTA 0 and CTA 1, of the columns; see Tc3Tile
     int32_t *vis;
 };
 
@@ -85,9 +85,17 @@ struct Tc3Params {
 // The units left over after the last whole wave are cut into one contiguous range of groups per CTA pair
 // ("stream-K"), so the tail costs every pair the same time whatever the number of tiles.  A segment is
 // the part of one unit that one pair computes: a whole unit, or a piece of a tail unit.
+// A pair tile: CTA r computes the 128 x 128 block (rows = inputs of block r ? xb : xa, columns = inputs of
+// block by).  Normal tiles hold blocks of the upper triangle as they are (row block <= column block).  A
+// TRANSPOSED tile holds blocks (x = by, y = xa) and (x = by, y = xb) of the triangle computed the other way round
+// (rows = the y inputs): this is how the blocks left over when a block column has an odd number of row blocks
+// are paired up -- as rows they differ, but transposed they all share the column block 0 -- instead of being
+// computed next to an idle CTA.  The epilogue conjugates and writes them transposed.  xb = 0xFFFF: no block.
+constexpr unsigned short TC3_TILE_TRANSPOSED = 1, TC3_NO_BLOCK = 0xFFFF;
+
 struct Tc3Seg {
     int u, f, slice;
-    ushort2 tile;
+    ushort4 tile;
     int first, cnt, len;   // groups [first, first + cnt) of the unit's len groups
     int t_begin, t_end;    // first sample of the segment; end of the unit's slice (<= T)
 };
@@ -205,10 +213,10 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             uint32_t ph = 0;
             while (tc3_next_segment(p, sit, sg)) {
                 const int f = sg.f;
-                const ushort2 tile = sg.tile;
+                const ushort4 tile = sg.tile;
                 const int t_begin = sg.t_begin;
-                const int xc = tile.x * 256 + (int)rank * 128;
-                const int yc = tile.y * 128 + (int)rank * 64;
+                const int xc = (int)(rank ? tile.y : tile.x) * 128;   // TC3_NO_BLOCK: out of bounds, TMA fills zeros
+                const int yc = tile.z * 128 + (int)rank * 64;
                 const int t_pad = t_begin + sg.cnt * T3_GROUP;   // whole groups of stages
                 for (int t = t_begin; t < t_pad; t += T3_ST) {
                     ptx::mbar_wait(pk_empty(st), ph ^ 1u);
@@ -365,10 +373,51 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             const bool raise_flag = !base_add && partial && last;
             int *flag = p.flags + 2 * sg.u + (int)rank;
             const int f = sg.f;
-            const ushort2 tile = sg.tile;
-            const int x0 = tile.x * 256 + (int)rank * 128, y0 = tile.y * 128;
+            const ushort4 tile = sg.tile;
+            const int x0 = (int)(rank ? tile.y : tile.x) * 128, y0 = tile.z * 128;   // rows and columns of the MMA
             const int xw = x0 + q * 32;
             const int x = x0 + row;
+            const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
+            if (tile.w & TC3_TILE_TRANSPOSED) {
+                // ---- transposed block: this thread's MMA row is the baseline's y, the MMA columns are its x.
+                // vis(x', y') = conj(D[y'][x']); for one column the 32 lanes of a warp hold consecutive y', which
+                // are consecutive in vis: every store instruction writes one contiguous 256-byte run.
+                ptx::mbar_wait_cluster(acc_full, acc_ph);
+                acc_ph ^= 1u;
+                ptx::tc_fence_after_sync();
+                if (wait_flag)
+                    while (ptx::ld_acquire_gpu(flag) != p.epoch) {
+                    }
+                const int yt = x;   // true y of this thread
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int col = 64 * h + 16 * c;
+                    const int xt0 = y0 + col;   // true x of the chunk's first column
+                    const bool skip = (xt0 > xw + 31) || (xt0 >= p.N) || (xw >= p.N);  // warp-uniform
+                    if (!skip) {
+                        uint32_t ir[16], rr[16], ri[16];
+                        ptx::tmem_ld16(trow + col, ir);
+                        ptx::tmem_ld16(trow + 128 + col, rr);
+                        ptx::tmem_ld16(trow + 256 + col, ri);
+                        ptx::tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int xt = xt0 + j;
+                            if (yt < p.N && xt <= yt) {
+                                const int re = (int)rr[j] >> 8;
+                                const int im = -((int)(ir[j] - ri[j]) >> 8);
+                                int2 *o = reinterpret_cast<int2 *>(p.vis) + (long long)f * Bn + (long long)xt * p.N -
+                                          (long long)xt * (xt - 1) / 2 + (yt - xt);
+                                if (add) { atomicAdd(&o->x, re); atomicAdd(&o->y, im); }
+                                else *o = make_int2(re, im);
+                            }
+                        }
+                    }
+                }
+                ptx::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
+            } else {
             // 8-byte index of (x, y0) in vis (formal when y0 < x: only its parity and offsets from it are used)
             const long long g0 = (long long)f * Bn + (long long)x * p.N - (long long)x * (x - 1) / 2 - x + y0;
             int2 *grow = reinterpret_cast<int2 *>(p.vis) + g0;
@@ -377,7 +426,6 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             ptx::mbar_wait_cluster(acc_full, acc_ph);
             acc_ph ^= 1u;
             ptx::tc_fence_after_sync();
-            const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int col = 64 * h + 16 * c;
@@ -425,6 +473,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                     if (add) ptx::bulk_reduce_add_s32(grow + jlo, srow + 8u * (par + jlo), 8u * (jhi - jlo));
                     else ptx::bulk_store(grow + jlo, srow + 8u * (par + jlo), 8u * (jhi - jlo));
                 }
+            }
             }
             ptx::bulk_commit();
             if (raise_flag) {
