@@ -32,8 +32,8 @@ if str(ROOT) not in sys.path:
 
 METRIC = "effective correlation TOPS (8 ops/CMAC/baseline) at N=2048; % of int8 TC peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of one corr_tc3_kernel launch on cfg3, from the ncu --set full
-# capture summarised in profiles/r01_tc3_ncu_summary.md (135.3 MB + 95.8 MB; algorithmic: 134.2 + 134.3 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = 231.1e6
+# capture summarised in profiles/r01_tc3_ncu_summary.md (136.4 MB + 98.7 MB; algorithmic: 134.2 + 134.3 MB)
+NCU_DRAM_BYTES_PER_LAUNCH = 235.1e6
 NOMINAL_INT8_TOPS = 4500.0  # dense int8 = 2x dense bf16 2250 (B200_PROFILING.md nominal table)
 
 
