@@ -66,31 +66,30 @@ corr_shift_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, con
         // (SH_THREADS is a multiple of 8, so a thread keeps its column group c for every row it handles)
         const int c = tid & 7;
         bool same = true;
+        int off[16];   // shared-memory offset of this thread's 16 inputs relative to output row 0 (loop invariant)
 #pragma unroll
-        for (int j = 1; j < 16; ++j) same = same && (slag[16 * c + j] == slag[16 * c]);
-        for (int idx = tid; idx < tcount * 8; idx += SH_THREADS) {
-            const int tr = idx >> 3;
-            if (c >= c16n) continue;
-            if (same) {
-                const int r = tr + hi - slag[16 * c];
-                *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) =
-                    *reinterpret_cast<const uint4 *>(tile + r * 128 + 16 * c);
-                continue;
-            }
-            uint32_t w[4];
+        for (int j = 0; j < 16; ++j) {
+            same = same && (slag[16 * c + j] == slag[16 * c]);
+            off[j] = (hi - slag[16 * c + j]) * 128 + 16 * c + j;
+        }
+        if (c < c16n) {
+            for (int tr = tid >> 3; tr < tcount; tr += SH_THREADS / 8) {
+                uint4 v;
+                if (same) {
+                    v = *reinterpret_cast<const uint4 *>(tile + tr * 128 + off[0]);
+                } else {
+                    const uint8_t *rowp = tile + tr * 128;
+                    uint32_t w[4];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                uint32_t acc = 0;
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int n = 16 * c + 4 * q + j;
-                    const int r = tr + hi - slag[n];
-                    acc |= (uint32_t)tile[r * 128 + n] << (8 * j);
+                    for (int q = 0; q < 4; ++q) {
+                        const uint32_t b0 = rowp[off[4 * q + 0]], b1 = rowp[off[4 * q + 1]];
+                        const uint32_t b2 = rowp[off[4 * q + 2]], b3 = rowp[off[4 * q + 3]];
+                        w[q] = __byte_perm(b0 | (b1 << 8), b2 | (b3 << 8), 0x5410);
+                    }
+                    v = make_uint4(w[0], w[1], w[2], w[3]);
                 }
-                w[q] = acc;
+                *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) = v;
             }
-            *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) =
-                make_uint4(w[0], w[1], w[2], w[3]);
         }
     } else {
         // ---- general path: one byte per thread-iteration straight from global memory
