@@ -222,6 +222,36 @@ def test_int32_headroom_edge(corr):
     assert (got[..., 0] == 128 * T).all() and (got[..., 1] == 0).all()
 
 
+@pytest.mark.parametrize("case", [(272, 3, 700, "TCGEN05"), (2048, 1, 300, "TCGEN05"), (400, 2, 520, "TCGEN05"),
+                                  (16, 9, 3000, "IMMA"), (64, 3, 1300, "IMMA"), (100, 2, 300, "DP4A"), (17, 3, 65, "DP4A")])
+def test_no_write_outside_the_output(corr, oracle, case):
+    # guard words on both sides of vis (and of the device input): every kernel, store / add / atomic modes,
+    # tiles and rows that hang over N, ragged T
+    import torch
+    N, F, T, path = case
+    packed = workloads.uniform_bytes(N, F, T, seed=N * 3 + T)
+    want = oracle.level1(packed)
+    G = 256   # guard ints (1 KB keeps vis 16-byte aligned)
+    for variant in (("3", "4") if path == "TCGEN05" else ("3",)):
+        import os
+        os.environ["CORR_TC_VARIANT"] = variant
+        try:
+            with corr.Plan(N, F, T, getattr(corr, "PATH_" + path)) as plan:
+                buf = torch.full((2 * G + plan.vis_elems,), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+                vis = buf[G:G + plan.vis_elems].view(F, plan.baselines, 2)
+                inbuf = torch.full((2048 + packed.size,), 0x88, dtype=torch.uint8, device="cuda")
+                dev = inbuf[1024:1024 + packed.size].view(T, F, N)
+                dev.copy_(torch.from_numpy(packed))
+                plan.execute(dev, vis)
+                plan.execute(dev, vis, accumulate=True)
+                torch.cuda.synchronize()
+                assert np.array_equal(vis.cpu().numpy(), 2 * want), (case, variant)
+                assert (buf[:G] == 0x5A5A5A5A).all() and (buf[G + plan.vis_elems:] == 0x5A5A5A5A).all(), (case, variant)
+                assert (inbuf[:1024] == 0x88).all() and (inbuf[1024 + packed.size:] == 0x88).all()
+        finally:
+            os.environ.pop("CORR_TC_VARIANT", None)
+
+
 def test_invalid_arguments(corr):
     for bad in [(0, 1, 1), (16, 0, 1), (16, 1, 0), (16, 1, 1 << 24)]:
         with pytest.raises(corr.CorrError):
