@@ -57,11 +57,13 @@ def main():
         out_bytes = vis.numel() * 4 * (2 if acc else 1)
         gbs = (N * F * T + out_bytes) / (ms * 1e-3) / 1e9
         rows.append((label, N, F, T, plan.info["path"], plan.info["slices"], plan.info["units"], ms,
-                     ops / (ms * 1e-3) / 1e12, gbs))
+                     ops / (ms * 1e-3) / 1e12, gbs, F * T / (ms * 1e-3) / 1e6))
         plan.close()
         del ins, vis
         torch.cuda.empty_cache()
-    hdr = ("shape", "N", "F", "T", "path", "slices", "units", "ms", "eff_TOPS", "HBM_GBs")
+    # Mmatrices_per_s: correlation matrices (one channel, one time step) per second, the unit of the paper's
+    # Fig. 4 upper panel (0.3318 M/s at N = 2048 on an R9 280X)
+    hdr = ("shape", "N", "F", "T", "path", "slices", "units", "ms", "eff_TOPS", "HBM_GBs", "Mmatrices_per_s")
     lines = [",".join(hdr)] + [",".join(f"{v:.4g}" if isinstance(v, float) else str(v) for v in r) for r in rows]
     print("\n".join(lines))
     if args.csv:
