@@ -235,6 +235,8 @@ def main():
     kernel_ms = ms_per_step  # one kernel launch per step; launch gaps are inside the figure
     achieved = eff_ops(N, F, T) / (kernel_ms * 1e-3) / 1e12
     path = plan.info["path"]
+    # the int8 ceiling of THIS device: a bare issue loop of the hot path's own tcgen05.mma.kind::i8 (~3 ms)
+    int8_measured = corr.corr_measure_int8_tops(20000)
     if path == corr.PATH_TCGEN05:
         variant = os.environ.get("CORR_TC_VARIANT", "3")
         kernel = {"1": "corr_tc_kernel", "2": "corr_tc2_kernel", "4": "corr_tc4_kernel"}.get(variant, "corr_tc3_kernel")
@@ -243,6 +245,7 @@ def main():
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == "cfg3" and kernel == "corr_tc3_kernel") else None,
             "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
             "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
+            "int8_issue_loop_tops": int8_measured, "frac_of_int8_issue_loop": achieved / int8_measured,
             "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
             "kernel": kernel, "kernel_ms": kernel_ms,
             "algorithmic_ops_per_launch": eff_ops(N, F, T),

@@ -135,6 +135,13 @@ int corr_execute_gated(corr_plan *plan, const uint8_t *packed_dev, const int32_t
 int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int32_t *lags_dev,
                     uint8_t *packed_out_dev, corr_stream_t stream);
 
+/* corr_measure_int8_tops -- measurement aid, not part of the correlation path: runs a bare issue loop of
+ * the hot path's own instruction (tcgen05.mma.cta_group::2.kind::i8, 256 x 128 x 32, A in TMEM, B in shared
+ * memory; `iters` x 4 MMAs per CTA pair, one pair per two SMs) on the current device's default stream,
+ * synchronises, and stores the achieved dense int8 TOPS (2 ops per multiply-add) in *tops_out (HOST pointer).
+ * This is the ceiling the roofline of section 8(d) is also reported against.  Returns CORR_OK or an error. */
+int corr_measure_int8_tops(int iters, double *tops_out);
+
 /* corr_plan_destroy -- free the plan and its device scratch.  NULL is a no-op. */
 void corr_plan_destroy(corr_plan *plan);
 

@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops")
 
 
 class CorrError(RuntimeError):
@@ -59,6 +59,8 @@ def load_library():
         lib.corr_count_tiles.restype = ci
         lib.corr_execute_gated.argtypes = [vp, vp, vp, ci, vp, ci, vp]
         lib.corr_execute_gated.restype = ci
+        lib.corr_measure_int8_tops.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
+        lib.corr_measure_int8_tops.restype = ci
         lib.corr_time_shift.argtypes = [ci, ci, ci, vp, vp, vp, vp]
         lib.corr_time_shift.restype = ci
         _lib = lib
@@ -96,6 +98,15 @@ def corr_execute_gated(plan: int, packed_dev_ptr: int, gate_host_ptr: int, G: in
                                            int(bool(accumulate_flag)), stream)
     if rc != 0:
         raise CorrError(f"corr_execute_gated -> {rc}: {_err()}")
+
+
+def corr_measure_int8_tops(iters: int = 20000) -> float:
+    """Dense int8 TOPS of a bare tcgen05.mma.kind::i8 issue loop on the current device (synchronises)."""
+    out = ctypes.c_double(0.0)
+    rc = load_library().corr_measure_int8_tops(iters, ctypes.byref(out))
+    if rc != 0:
+        raise CorrError(f"corr_measure_int8_tops -> {rc}: {_err()}")
+    return out.value
 
 
 def corr_time_shift(N: int, F: int, T: int, packed_in_ptr: int, lags_ptr: int, packed_out_ptr: int, stream: int) -> None:

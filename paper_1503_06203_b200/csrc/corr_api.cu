@@ -16,6 +16,7 @@
 #include "corr_dp4a.cuh"
 #include "corr_gate.cuh"
 #include "corr_imma.cuh"
+#include "corr_peak.cuh"
 #include "corr_shift.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
@@ -421,6 +422,40 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
 }
 
 corr_plan *corr_plan_create(int N, int F, int T) { return corr_plan_create_ex(N, F, T, CORR_PATH_AUTO); }
+
+int corr_measure_int8_tops(int iters, double *tops_out)
+{
+    if (iters < 1 || !tops_out) {
+        set_err("corr_measure_int8_tops: need iters >= 1 and a result pointer");
+        return CORR_ERR_INVALID_ARG;
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDevice(&dev), CORR_ERR_CUDA);
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev), CORR_ERR_CUDA);
+    if (prop.major != 10) {
+        set_err("corr_measure_int8_tops: needs an sm_100 device");
+        return CORR_ERR_UNSUPPORTED;
+    }
+    CUDA_TRY(cudaFuncSetAttribute(corr::corr_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::PK_SMEM_BYTES),
+             CORR_ERR_CUDA);
+    const int grid = prop.multiProcessorCount / 2 * 2;
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0), CORR_ERR_CUDA);
+    CUDA_TRY(cudaEventCreate(&e1), CORR_ERR_CUDA);
+    corr::corr_peak_kernel<<<grid, corr::PK_THREADS, corr::PK_SMEM_BYTES>>>(iters / 8 + 1);   // warm-up
+    CUDA_TRY(cudaEventRecord(e0), CORR_ERR_CUDA);
+    corr::corr_peak_kernel<<<grid, corr::PK_THREADS, corr::PK_SMEM_BYTES>>>(iters);
+    CUDA_TRY(cudaEventRecord(e1), CORR_ERR_CUDA);
+    CUDA_TRY(cudaEventSynchronize(e1), CORR_ERR_CUDA);
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1), CORR_ERR_CUDA);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    // per CTA pair and iteration: 4 MMAs of 256 x 128 x 32 multiply-adds
+    *tops_out = (double)(grid / 2) * iters * 4.0 * 2.0 * 256.0 * 128.0 * 32.0 / (ms * 1e-3) / 1e12;
+    return CORR_OK;
+}
 
 int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int32_t *lags_dev, uint8_t *packed_out_dev,
                     corr_stream_t stream_)
