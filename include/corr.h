@@ -91,7 +91,10 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path);
  *               to).
  *   stream      CUDA stream the work is enqueued on.
  * Returns CORR_OK or an error code; errors found at enqueue time are returned here, later
- * device faults surface at the caller's own synchronisation.  The caller owns both buffers. */
+ * device faults surface at the caller's own synchronisation.  The caller owns both buffers.
+ * A plan holds per-call state (the tensor map of the last input pointer, the schedule's flags and
+ * call counter, scratch buffers): calls on ONE plan must be issued from one host thread at a time
+ * and onto one stream (or streams the caller orders); use one plan per concurrent stream. */
 int corr_execute(corr_plan *plan, const uint8_t *packed_dev, int32_t *vis_dev,
                  int accumulate_flag, corr_stream_t stream);
 
