@@ -47,10 +47,8 @@ template <int NT16> struct ImmaCfg {
     static constexpr int SETS = NT16 / MS;                     // m-tiles per warp (1, 2, 2)
     static constexpr int KS = (NT16 == 1) ? 2 : (NT16 == 2) ? 4 : 2;   // K-split
     static constexpr int WARPS = FB * MS * KS;                 // consumer warps (16, 16, 8)
-    // TMA producer: a warp of its own (measured 7 % faster than thread 0 issuing the loads between its
-    // consumer iterations; kept as an option because 17 warps cap a thread at 96 registers)
-    static constexpr bool SEP = true;
-    static constexpr int THREADS = 32 * (WARPS + (SEP ? 1 : 0));
+    // + the TMA producer warp (measured 7 % faster than thread 0 issuing the loads between its consumer iterations)
+    static constexpr int THREADS = 32 * (WARPS + 1);
 };
 
 struct ImmaParams {
@@ -107,7 +105,7 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
         ptx::prefetch_tmap(&tmap);
         for (int s = 0; s < IM_STAGES; ++s) {
             ptx::mbar_init(full(s), 1);
-            ptx::mbar_init(empty(s), C::WARPS);
+            ptx::mbar_init(empty(s), C::WARPS / C::KS);   // the warps that own the stage (see the K-split below)
         }
         ptx::fence_mbar_init();
     }
@@ -128,8 +126,6 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     const int ks = warp / (C::FB * C::MS);          // K-split index
     const int f = strip * C::FB + ch;
 
-    // TMA producer = thread 0, interleaved with its consumer work: stage it + IM_STAGES - 1 is requested at
-    // the top of iteration it (its ring slot was released by every warp in iteration it - 1)
     auto produce = [&](int j) {
         if (j < nstages) {
             const int sj = j % IM_STAGES;
@@ -138,26 +134,23 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
             ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj), strip * 128, t_begin + j * IM_ROWS);
         }
     };
-    if (C::SEP && warp == C::WARPS) {
+    if (warp == C::WARPS) {
+        // ===================== TMA producer =====================
         if (lane == 0)
             for (int j = 0; j < nstages; ++j) produce(j);
     } else {
         // ===================== consumers =====================
-        if (!C::SEP && threadIdx.x == 0)
-            for (int j = 0; j < IM_STAGES - 1; ++j) produce(j);
         const uint32_t c16 = (uint32_t)(ch * N) >> 4;   // first 16-byte chunk of this channel in a 128-byte row
-        for (int it = 0; it < nstages; ++it) {
+        // K-split by STAGE: warp ks takes the stages it with it % KS == ks, whole.  The warps of one SM
+        // sub-partition (same channel, different ks) then wait on different barriers and drift apart, so the
+        // load / unpack phase of one overlaps the MMA phase of another instead of all four moving in lockstep.
+        for (int it = ks; it < nstages; it += C::KS) {
             const int s = it % IM_STAGES;
-            if (!C::SEP) {
-                if (threadIdx.x == 0) produce(it + IM_STAGES - 1);
-                __syncwarp();
-            }
             ptx::mbar_wait(full(s), (uint32_t)(it / IM_STAGES) & 1u);
             const uint32_t stage = base + s * IM_STAGE_BYTES;
             if (f < p.F) {
 #pragma unroll
-                for (int kk = 0; kk < IM_ROWS / 32 / C::KS; ++kk) {
-                    const int kb = ks + C::KS * kk;                       // K-block of 32 samples inside the stage
+                for (int kb = 0; kb < IM_ROWS / 32; ++kb) {             // K-blocks of 32 samples of the stage
                     const int valid = t_end - (t_begin + it * IM_ROWS + 32 * kb);   // samples of this K-block inside the chunk
                     if (valid <= 0) continue;
                     const uint32_t r = 32u * kb + lane;                   // ldmatrix row of this lane (time sample)
