@@ -92,6 +92,8 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path);
  *   stream      CUDA stream the work is enqueued on.
  * Returns CORR_OK or an error code; errors found at enqueue time are returned here, later
  * device faults surface at the caller's own synchronisation.  The caller owns both buffers.
+ * The call only enqueues kernels and memsets, so it may be captured into a CUDA graph and replayed
+ * (with the buffers it was captured with).
  * A plan holds per-call state (the tensor map of the last input pointer, the schedule's flags and
  * call counter, scratch buffers): calls on ONE plan must be issued from one host thread at a time
  * and onto one stream (or streams the caller orders); use one plan per concurrent stream. */

@@ -375,8 +375,8 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->groups_last = (T - (p->slices - 1) * p->t_per_slice + corr::T3_GROUP - 1) / corr::T3_GROUP;
         p->total_groups = units0 * ((long long)(p->slices - 1) * p->groups_full + p->groups_last);
         p->grid = 2 * (int)std::min<long long>(p->total_groups, p->sm_count / 2);
-        if (cudaMalloc(&p->flags_dev, 2 * (size_t)p->num_units * sizeof(int)) != cudaSuccess ||
-            cudaMemset(p->flags_dev, 0, 2 * (size_t)p->num_units * sizeof(int)) != cudaSuccess) {
+        if (cudaMalloc(&p->flags_dev, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess ||
+            cudaMemset(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess) {
             set_err("corr_plan_create: device allocation of the schedule flags failed: %s",
                     cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
@@ -621,7 +621,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.groups_last = p->groups_last;
             prm.total_groups = p->total_groups;
             if (p->epoch == 0x7fffffff) {   // the call counter wraps: forget every flag of the previous era
-                CUDA_TRY(cudaMemsetAsync(p->flags_dev, 0, 2 * (size_t)p->num_units * sizeof(int), stream), CORR_ERR_CUDA);
+                CUDA_TRY(cudaMemsetAsync(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int), stream), CORR_ERR_CUDA);
                 p->epoch = 0;
             }
             prm.epoch = ++p->epoch;

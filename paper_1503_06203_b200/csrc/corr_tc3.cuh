@@ -74,7 +74,8 @@ struct Tc3Params {
     int groups_last;   // ... in the last slice of a tile
     long long total_groups;  // over all units
     int epoch;         // corr_execute call counter of the plan, > 0
-    int *flags;        // [num_units][2]: == epoch once the storing segment of (unit, CTA rank) is in memory
+    int *flags;        // [num_units][2]: == epoch once the storing segment of (unit, CTA rank) is in memory;
+                       // [2 * num_units]: CTAs that have finished (the last one clears the array for the next launch)
     const ushort4 *tiles;  // (xa, xb, by, flags): 128-blocks of the rows of CTA 0 and CTA 1, of the columns; see Tc3Tile
     int32_t *vis;
 };
@@ -490,6 +491,17 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     ptx::tc_fence_before_sync();
     ptx::cluster_sync();  // no CTA of the pair may exit while its peer still reads its smem / barriers
     if (warp == 1) ptx::tmem_dealloc<2>(tmem, 512);
+    // The last CTA to get here clears the flags, so that a launch replayed with the same call counter (a
+    // captured CUDA graph) starts from a clean array: nobody reads a flag after its own CTA has counted itself.
+    if (threadIdx.x == 0) {
+        __threadfence();
+        int *done = p.flags + 2 * p.num_units;
+        if (atomicAdd(done, 1) == (int)gridDim.x - 1) {
+            for (int i = 0; i < 2 * p.num_units; ++i) p.flags[i] = 0;
+            __threadfence();
+            *done = 0;
+        }
+    }
 }
 
 }  // namespace corr

@@ -171,6 +171,31 @@ def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
         assert np.array_equal(got, oracle.level1(packed)), (variant, hex(byte))
 
 
+def test_cuda_graph_replay(corr, oracle):
+    # corr_execute only enqueues (kernels + memsets), so it can be captured; a replayed launch carries the
+    # same call counter, which the schedule's flags must survive (the last CTA clears them)
+    import torch
+    for (N, F, T) in [(256, 2, 20000), (1024, 3, 700), (64, 5, 70000)]:   # cut units / whole waves + tail / chunked atomics
+        packed = workloads.iid_gaussian(N, F, T, seed=N + F)
+        want = oracle.level1(packed)
+        with corr.Plan(N, F, T) as plan:
+            dev = torch.from_numpy(packed).cuda()
+            vis = plan.new_vis()
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                plan.execute(dev, vis, stream=side)          # warm-up outside the graph (tensor map, attributes)
+                side.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    plan.execute(dev, vis, stream=side)
+            for rep in range(3):
+                vis.fill_(-559038737)
+                g.replay()
+                torch.cuda.synchronize()
+                assert np.array_equal(vis.cpu().numpy(), want), (N, F, T, rep)
+
+
 def test_execute_host(corr, oracle):
     import torch
     packed = workloads.iid_gaussian(160, 2, 700, seed=9)
