@@ -171,6 +171,35 @@ def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
         assert np.array_equal(got, oracle.level1(packed)), (variant, hex(byte))
 
 
+def _fuzz_cases(seed, count):
+    rng = np.random.default_rng(seed)
+    for _ in range(count):
+        kind = rng.integers(0, 4)
+        if kind == 0:
+            N = int(rng.choice([16, 32, 64]))                      # warp-MMA path
+        elif kind == 1:
+            N = int(rng.integers(1, 200))                          # dp4a path (or tcgen05 when N % 16 == 0, N >= 96)
+        else:
+            N = 16 * int(rng.integers(6, 90))                      # tcgen05 path: odd / even block counts, ragged blocks
+        F = int(rng.integers(1, 6))
+        T = int(rng.choice([1, 63, 64, 255, 256, 257, 1000, 3000, 5000])) + int(rng.integers(0, 3))
+        if N > 700:
+            T = min(T, 1100)
+        yield N, F, T, bool(rng.integers(0, 2)), int(rng.integers(0, 1 << 30))
+
+
+def test_fuzz_shapes(corr, oracle):
+    # random shapes through the automatic path choice, overwrite then (sometimes) accumulate, stale output
+    for N, F, T, acc, seed in _fuzz_cases(20240607, 40):
+        packed = workloads.uniform_bytes(N, F, T, seed=seed)
+        want = oracle.level1(packed)
+        got, info = _run(corr, packed, prefill=-559038737)
+        assert np.array_equal(got, want), (N, F, T, info)
+        if acc:
+            both, _ = _run(corr, packed, accumulate_into=got.copy())
+            assert np.array_equal(both, 2 * want), (N, F, T, info, "accumulate")
+
+
 def test_cuda_graph_replay(corr, oracle):
     # corr_execute only enqueues (kernels + memsets), so it can be captured; a replayed launch carries the
     # same call counter, which the schedule's flags must survive (the last CTA clears them)
