@@ -12,8 +12,9 @@
 // thread assembles 16 output bytes from the rows its inputs' lags select and writes them with one 16-byte
 // store (a single 16-byte shared-memory load when the 16 inputs share one lag, the common case of a few
 // cable lengths).  Read amplification (SH_TB + spread) / SH_TB, spread = max lag - min lag over the 128 inputs.  When
-// the spread does not fit in shared memory, or N is not a multiple of 16, the CTA gathers byte by byte from
-// global memory instead (correct, slow).
+// the spread does not fit, the CTA goes through its inputs 16 at a time with a 16-byte-wide window that can be
+// eight times longer (spreads up to 4480 samples); beyond that, or when N is not a multiple of 16, it gathers
+// byte by byte from global memory (correct, slow).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -89,6 +90,50 @@ corr_shift_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, con
                     v = make_uint4(w[0], w[1], w[2], w[3]);
                 }
                 *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) = v;
+            }
+        }
+    } else if ((N & 15) == 0) {
+        // ---- wide spread: one group of 16 inputs at a time, so the window is 16 bytes wide and can be
+        //      8 x longer (spreads up to SH_MAX_ROWS * 8 - SH_TB rows inside a group of 16 inputs)
+        const int c16n = ncols >> 4;
+        for (int c = 0; c < c16n; ++c) {
+            int glo = 0x7fffffff, ghi = (int)0x80000000;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) { glo = min(glo, slag[16 * c + j]); ghi = max(ghi, slag[16 * c + j]); }
+            const long long grows = (long long)SH_TB + (long long)ghi - (long long)glo;
+            if (grows <= SH_MAX_ROWS * 8) {
+                __syncthreads();   // the previous group's window is no longer read
+                for (int r = tid; r < (int)grows; r += SH_THREADS) {
+                    const long long tin = (long long)t0 - ghi + r;
+                    uint4 v = make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
+                    if (tin >= 0 && tin < T)
+                        v = __ldg(reinterpret_cast<const uint4 *>(in + ((size_t)tin * F + f) * (size_t)N + n0 + 16 * c));
+                    *reinterpret_cast<uint4 *>(tile + r * 16) = v;
+                }
+                __syncthreads();
+                for (int tr = tid; tr < tcount; tr += SH_THREADS) {
+                    uint32_t w[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        uint32_t acc = 0;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const int n = 4 * q + j;
+                            acc |= (uint32_t)tile[(tr + ghi - slag[16 * c + n]) * 16 + n] << (8 * j);
+                        }
+                        w[q] = acc;
+                    }
+                    *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) =
+                        make_uint4(w[0], w[1], w[2], w[3]);
+                }
+            } else {
+                for (int idx = tid; idx < tcount * 16; idx += SH_THREADS) {
+                    const int tr = idx >> 4, n = 16 * c + (idx & 15);
+                    const long long tin = (long long)t0 + tr - slag[n];
+                    uint8_t b = 0x88;
+                    if (tin >= 0 && tin < T) b = in[((size_t)tin * F + f) * (size_t)N + n0 + n];
+                    out[((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + n] = b;
+                }
             }
         }
     } else {
