@@ -222,12 +222,12 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         else if (force && !strcmp(force, "imma"))
             path = CORR_PATH_IMMA;
         else
-            path = (N == 16 || N == 32 || N == 64) ? CORR_PATH_IMMA
-                   : (N % 16 == 0 && N >= 96)      ? CORR_PATH_TCGEN05
-                                                   : CORR_PATH_DP4A;
+            path = (N == 16 || N == 32 || N == 48 || N == 64) ? CORR_PATH_IMMA
+                   : (N % 16 == 0)                            ? CORR_PATH_TCGEN05   // measured 3-10x the dp4a kernel from N = 80 up
+                                                              : CORR_PATH_DP4A;
     }
-    if (path == CORR_PATH_IMMA && !(N == 16 || N == 32 || N == 64)) {
-        set_err("corr_plan_create: the warp-MMA path takes N = 16, 32 or 64, got N=%d", N);
+    if (path == CORR_PATH_IMMA && !(N == 16 || N == 32 || N == 48 || N == 64)) {
+        set_err("corr_plan_create: the warp-MMA path takes N = 16, 32, 48 or 64, got N=%d", N);
         return nullptr;
     }
     if (path == CORR_PATH_TCGEN05 && N % 16 != 0) {
@@ -258,11 +258,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         const int strips = (F + fb - 1) / fb;
         cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
         int occ = 1;
         if (e == cudaSuccess) {
             if (N == 16) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<1>, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES);
             else if (N == 32) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<2>, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES);
+            else if (N == 48) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<3>, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES);
             else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<4>, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES);
         }
         if (e != cudaSuccess || occ < 1) {
@@ -563,6 +565,8 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             corr::corr_imma_kernel<1><<<grid, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
         else if (p->N == 32)
             corr::corr_imma_kernel<2><<<grid, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
+        else if (p->N == 48)
+            corr::corr_imma_kernel<3><<<grid, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
         else
             corr::corr_imma_kernel<4><<<grid, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
     } else if (p->path == CORR_PATH_DP4A) {

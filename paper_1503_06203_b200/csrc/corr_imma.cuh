@@ -1,4 +1,4 @@
-// corr_imma.cuh -- step S4' of the hot path for N = 16, 32, 64: warp-level int8 tensor-core
+// corr_imma.cuh -- step S4' of the hot path for N = 16, 32, 48, 64: warp-level int8 tensor-core
 // MMA (mma.sync.m16n8k32.s8) on whole channels, fed by TMA.
 //
 // Why not dp4a here: measured on B200, IDP.4A issues 64 lanes/clk/SM = 17.5 T dp4a/s, i.e. 140
@@ -42,11 +42,12 @@ constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 256;
 
 template <int NT16> struct ImmaCfg {
     static constexpr int N = 16 * NT16;
-    static constexpr int FB = 128 / N;                         // channels per strip
+    static constexpr int FB = 128 / N;                         // whole channels per 128-byte strip (8, 4, 2, 2)
+    static constexpr int STRIP = FB * N;                       // bytes between strips (N = 48: 96, boxes overlap by 32)
     static constexpr int MS = (NT16 == 4) ? 2 : 1;             // warps that share a channel's m-tiles
-    static constexpr int SETS = NT16 / MS;                     // m-tiles per warp (1, 2, 2)
-    static constexpr int KS = (NT16 == 1) ? 2 : (NT16 == 2) ? 4 : 2;   // K-split
-    static constexpr int WARPS = FB * MS * KS;                 // consumer warps (16, 16, 8)
+    static constexpr int SETS = NT16 / MS;                     // m-tiles per warp (1, 2, 3, 2)
+    static constexpr int KS = (NT16 == 1) ? 2 : (NT16 == 4) ? 2 : 4;   // K-split
+    static constexpr int WARPS = FB * MS * KS;                 // consumer warps (16, 16, 8, 8)
     // + the TMA producer warp (measured 7 % faster than thread 0 issuing the loads between its consumer iterations)
     static constexpr int THREADS = 32 * (WARPS + 1);
 };
@@ -131,7 +132,7 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
             const int sj = j % IM_STAGES;
             ptx::mbar_wait(empty(sj), ((uint32_t)(j / IM_STAGES) & 1u) ^ 1u);
             ptx::mbar_arrive_expect_tx(full(sj), IM_STAGE_BYTES);
-            ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj), strip * 128, t_begin + j * IM_ROWS);
+            ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj), strip * C::STRIP, t_begin + j * IM_ROWS);
         }
     };
     if (warp == C::WARPS) {
@@ -180,6 +181,9 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
                     if constexpr (NT16 == 4) {
                         if (ms == 0) { imma_mtile<4, 0, 0, 2>(pr, pi, re, ir); imma_mtile<4, 3, 1, 2>(pr, pi, re, ir); }
                         else         { imma_mtile<4, 1, 0, 2>(pr, pi, re, ir); imma_mtile<4, 2, 1, 2>(pr, pi, re, ir); }
+                    } else if constexpr (NT16 == 3) {
+                        imma_mtile<3, 0, 0, 3>(pr, pi, re, ir); imma_mtile<3, 1, 1, 3>(pr, pi, re, ir);
+                        imma_mtile<3, 2, 2, 3>(pr, pi, re, ir);
                     } else if constexpr (NT16 == 2) {
                         imma_mtile<2, 0, 0, 2>(pr, pi, re, ir); imma_mtile<2, 1, 1, 2>(pr, pi, re, ir);
                     } else {

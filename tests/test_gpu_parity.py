@@ -65,7 +65,7 @@ def test_tcgen05_small_shapes(corr, oracle, N):
             assert np.array_equal(got, oracle.level1(packed)), (N, F, T)
 
 
-@pytest.mark.parametrize("N", [16, 32, 64])
+@pytest.mark.parametrize("N", [16, 32, 48, 64])
 def test_imma_small_n(corr, oracle, N):
     # warp-MMA path (whole channels per CTA): ragged T, F not a multiple of the channels per strip,
     # several time chunks (atomic accumulation), stale output, accumulate flag, extreme bytes
@@ -90,7 +90,7 @@ def test_imma_small_n(corr, oracle, N):
         packed = np.full((5000, 3, N), byte, np.uint8)
         got, _ = _run(corr, packed, corr.PATH_IMMA)
         assert np.array_equal(got, oracle.level1(packed)), (N, hex(byte))
-    auto, info = _run(corr, small)                                  # AUTO picks this path for N = 16, 32, 64
+    auto, info = _run(corr, small)                                  # AUTO picks this path for N = 16, 32, 48, 64
     assert info["path"] == corr.PATH_IMMA and np.array_equal(auto, w2)
 
 
@@ -313,7 +313,7 @@ def test_invalid_arguments(corr):
     with pytest.raises(corr.CorrError):
         corr.corr_plan_create(100, 1, 64, corr.PATH_TCGEN05)   # N % 16 != 0
     with pytest.raises(corr.CorrError):
-        corr.corr_plan_create(48, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N = 16, 32, 64 only
+        corr.corr_plan_create(80, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N = 16, 32, 48, 64 only
 
 
 # ------------------------------------------------------------------ the five BASELINE.json configs
