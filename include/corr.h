@@ -60,8 +60,8 @@ enum {
 enum {
     CORR_PATH_AUTO = 0,  /* library chooses from (N, F, T) */
     CORR_PATH_DP4A = 1,  /* CUDA-core dp4a kernels; any N (small-N path) */
-    CORR_PATH_TCGEN05 = 2, /* TMA + tcgen05 int8 MMA, int32 accumulators in TMEM; needs N % 16 == 0 */
-    CORR_PATH_IMMA = 3     /* TMA + warp-level int8 MMA on whole channels; N = 16, 32, 48 or 64 (small-N path) */
+    CORR_PATH_TCGEN05 = 2, /* TMA + tcgen05 int8 MMA, int32 accumulators in TMEM; any N (padded copy if N % 16 != 0) */
+    CORR_PATH_IMMA = 3     /* TMA + warp-level int8 MMA on whole channels; N <= 64 (small-N path) */
 };
 
 /* corr_plan_create -- validate the shape, choose the path, build the triangular tile schedule
@@ -70,8 +70,9 @@ enum {
  *   F  number of frequency channels,       F >= 1
  *   T  time samples per corr_execute call, 1 <= T <= 16 777 215
  * Returns NULL on failure; the reason is in corr_last_error().
- * Automatic choice: N = 16, 32, 48, 64 -> CORR_PATH_IMMA; any other N % 16 == 0 -> CORR_PATH_TCGEN05;
- * everything else -> CORR_PATH_DP4A.  Testing aids (environment, read at plan creation):
+ * Automatic choice: N <= 64 -> CORR_PATH_IMMA, larger N -> CORR_PATH_TCGEN05.  When N % 16 != 0 these
+ * two paths first copy the stream to a plan-owned buffer padded to the next multiple of 16 inputs
+ * (TMA strides); CORR_PATH_DP4A takes any N without a copy and is only used on request.  Testing aids (environment, read at plan creation):
  * CORR_FORCE_PATH=dp4a|tcgen05|imma overrides the choice; CORR_TC_VARIANT=1|2|3|4 selects the
  * tcgen05 kernel (default 3; 4 = three products per complex MAC with the Eq. 3 offset
  * correction). */

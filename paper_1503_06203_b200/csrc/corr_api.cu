@@ -79,6 +79,8 @@ int count_tiles(int N, int tx, int ty)
 
 struct corr_plan {
     int N, F, T, path;
+    int n_pad;         // N rounded up to a multiple of 16: the width of the stream the TMA-fed kernels read
+    uint8_t *pad_buf;  // T*F*n_pad bytes when n_pad != N (corr_pad_kernel)
     int sm_count;
     // schedule
     int tile;          // tile edge (square tiles)
@@ -156,6 +158,7 @@ int corr_plan_info(const corr_plan *p, int info[8])
 void corr_plan_destroy(corr_plan *p)
 {
     if (!p) return;
+    if (p->pad_buf) cudaFree(p->pad_buf);
     if (p->tiles_dev) cudaFree(p->tiles_dev);
     if (p->tiles4_dev) cudaFree(p->tiles4_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
@@ -213,6 +216,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
                 prop.major, prop.minor);
         return nullptr;
     }
+    const int n_pad = (N + 15) / 16 * 16;   // N % 16 != 0: the TMA-fed paths read a zero-padded copy of the stream
     if (path == CORR_PATH_AUTO) {
         const char *force = getenv("CORR_FORCE_PATH");
         if (force && !strcmp(force, "dp4a"))
@@ -222,16 +226,10 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         else if (force && !strcmp(force, "imma"))
             path = CORR_PATH_IMMA;
         else
-            path = (N == 16 || N == 32 || N == 48 || N == 64) ? CORR_PATH_IMMA
-                   : (N % 16 == 0)                            ? CORR_PATH_TCGEN05   // measured 3-10x the dp4a kernel from N = 80 up
-                                                              : CORR_PATH_DP4A;
+            path = (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;   // both measured 3-10x the dp4a kernel
     }
-    if (path == CORR_PATH_IMMA && !(N == 16 || N == 32 || N == 48 || N == 64)) {
-        set_err("corr_plan_create: the warp-MMA path takes N = 16, 32, 48 or 64, got N=%d", N);
-        return nullptr;
-    }
-    if (path == CORR_PATH_TCGEN05 && N % 16 != 0) {
-        set_err("corr_plan_create: the tcgen05 path needs N %% 16 == 0 (TMA row stride), got N=%d", N);
+    if (path == CORR_PATH_IMMA && n_pad > 64) {
+        set_err("corr_plan_create: the warp-MMA path takes N <= 64, got N=%d", N);
         return nullptr;
     }
 
@@ -242,6 +240,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     }
     memset(p, 0, sizeof(*p));
     p->N = N;
+    p->n_pad = n_pad;
     p->F = F;
     p->T = T;
     p->path = path;
@@ -254,7 +253,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             delete p;
             return nullptr;
         }
-        const int fb = 128 / N;
+        const int fb = 128 / n_pad;
         const int strips = (F + fb - 1) / fb;
         cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
@@ -262,9 +261,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (e == cudaSuccess) e = cudaFuncSetAttribute(corr::corr_imma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
         int occ = 1;
         if (e == cudaSuccess) {
-            if (N == 16) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<1>, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES);
-            else if (N == 32) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<2>, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES);
-            else if (N == 48) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<3>, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES);
+            if (n_pad == 16) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<1>, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES);
+            else if (n_pad == 32) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<2>, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES);
+            else if (n_pad == 48) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<3>, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES);
             else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<4>, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES);
         }
         if (e != cudaSuccess || occ < 1) {
@@ -288,7 +287,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->tiles_per_f = 1;
         p->num_units = strips * p->slices;
         p->grid = p->num_units;
-        p->kernels_per_exec = 1;
+        p->kernels_per_exec = (n_pad != N) ? 2 : 1;
         return p;
     }
 
@@ -301,6 +300,12 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     if (path == CORR_PATH_TCGEN05) {
         const char *v = getenv("CORR_TC_VARIANT");
         p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : (v && !strcmp(v, "4")) ? 4 : 3;
+        if (p->variant != 3 && n_pad != N) {
+            set_err("corr_plan_create: CORR_TC_VARIANT=%d needs N %% 16 == 0 (only the default kernel reads a padded stream), got N=%d",
+                    p->variant, N);
+            delete p;
+            return nullptr;
+        }
     }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
@@ -370,7 +375,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->grid = (path == CORR_PATH_DP4A) ? p->num_units
               : (p->variant >= 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
                                   : std::min(p->num_units, p->sm_count);
-    p->kernels_per_exec = (p->variant == 4) ? 2 : 1;  // tc4: corr_sums_kernel + corr_tc4_kernel
+    p->kernels_per_exec = ((p->variant == 4) ? 2 : 1) + ((path != CORR_PATH_DP4A && n_pad != N) ? 1 : 0);  // tc4: + corr_sums_kernel; + corr_pad_kernel
     p->aligned = (N % 4 == 0) ? 1 : 0;
     if (p->variant == 3) {
         p->groups_full = p->t_per_slice / corr::T3_GROUP;
@@ -492,8 +497,8 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     if (p->tmap_ptr == packed_dev) return CORR_OK;
     if (p->path == CORR_PATH_IMMA) {
         // packed[T][F][N] as a byte matrix, innermost first: (F*N, T), row stride F*N bytes
-        const cuuint64_t dims2[2] = {(cuuint64_t)p->F * (cuuint64_t)p->N, (cuuint64_t)p->T};
-        const cuuint64_t strides2[1] = {(cuuint64_t)p->F * (cuuint64_t)p->N};
+        const cuuint64_t dims2[2] = {(cuuint64_t)p->F * (cuuint64_t)p->n_pad, (cuuint64_t)p->T};
+        const cuuint64_t strides2[1] = {(cuuint64_t)p->F * (cuuint64_t)p->n_pad};
         const cuuint32_t box2[2] = {128u, (cuuint32_t)corr::IM_ROWS};
         const cuuint32_t estr2[2] = {1u, 1u};
         CUresult r2 = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(packed_dev), dims2,
@@ -507,8 +512,8 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
         return CORR_OK;
     }
     // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
-    const cuuint64_t dims[3] = {(cuuint64_t)p->N, (cuuint64_t)p->F, (cuuint64_t)p->T};
-    const cuuint64_t strides[2] = {(cuuint64_t)p->N, (cuuint64_t)p->F * (cuuint64_t)p->N};
+    const cuuint64_t dims[3] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F, (cuuint64_t)p->T};
+    const cuuint64_t strides[2] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F * (cuuint64_t)p->n_pad};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const int st = (p->variant == 4) ? corr::T4_ST : (p->variant == 3) ? corr::T3_ST : (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
@@ -536,11 +541,20 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         set_err("corr_execute: NULL plan or buffer");
         return CORR_ERR_INVALID_ARG;
     }
-    if ((reinterpret_cast<uintptr_t>(packed_dev) & 15u) || (reinterpret_cast<uintptr_t>(vis_dev) & 7u)) {
+    const bool padded = (p->path != CORR_PATH_DP4A && p->n_pad != p->N);
+    if ((!padded && (reinterpret_cast<uintptr_t>(packed_dev) & 15u)) || (reinterpret_cast<uintptr_t>(vis_dev) & 7u)) {
         set_err("corr_execute: packed_dev must be 16-byte aligned and vis_dev 8-byte aligned");
         return CORR_ERR_INVALID_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (padded) {
+        // N % 16 != 0: the TMA-fed kernels read a copy of the stream padded to n_pad inputs with stored zeros
+        const long long rows = (long long)p->T * p->F;
+        if (!p->pad_buf) CUDA_TRY(cudaMalloc(&p->pad_buf, (size_t)rows * p->n_pad), CORR_ERR_ALLOC);
+        corr::corr_pad_kernel<<<8 * p->sm_count, 256, 0, stream>>>(packed_dev, p->pad_buf, p->N, p->n_pad, rows);
+        CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+        packed_dev = p->pad_buf;
+    }
     int out_mode;
     if (p->slices > 1) {
         out_mode = corr::OUT_ATOMIC;
@@ -561,11 +575,11 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         prm.out_mode = out_mode;
         prm.vis = vis_dev;
         dim3 grid((unsigned)(p->num_units / p->slices), (unsigned)p->slices);
-        if (p->N == 16)
+        if (p->n_pad == 16)
             corr::corr_imma_kernel<1><<<grid, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
-        else if (p->N == 32)
+        else if (p->n_pad == 32)
             corr::corr_imma_kernel<2><<<grid, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
-        else if (p->N == 48)
+        else if (p->n_pad == 48)
             corr::corr_imma_kernel<3><<<grid, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);
         else
             corr::corr_imma_kernel<4><<<grid, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES, stream>>>(p->tmap, prm);

@@ -220,19 +220,50 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     }
     __syncthreads();
 
-    // ---- S5: form (Re, Im), keep x <= y, write
-    const size_t B = (size_t)N * (N + 1) / 2;
+    // ---- S5: form (Re, Im), keep x <= y, write.  p.N is the number of inputs the caller has (the stream may be
+    //      padded to the next multiple of 16 with zero samples): it decides the layout of vis.
+    const int NL = p.N;
+    const size_t B = (size_t)NL * (NL + 1) / 2;
     for (int i = threadIdx.x; i < C::FB * N * N; i += C::THREADS) {
         const int c = i / (N * N), x = (i / N) % N, y = i % N;
         const int fo = strip * C::FB + c;
-        if (fo >= p.F || y < x) continue;
+        if (fo >= p.F || y < x || y >= NL) continue;
         const int *rre = red + (c * 2 + 0) * N * N, *rir = red + (c * 2 + 1) * N * N;
         const int vre = rre[x * N + y] >> 8;
         const int vim = (rir[x * N + y] - rir[y * N + x]) >> 8;
-        int32_t *o = p.vis + 2 * ((size_t)fo * B + baseline_index(N, x, y));
+        int32_t *o = p.vis + 2 * ((size_t)fo * B + baseline_index(NL, x, y));
         if (p.out_mode == OUT_STORE) { o[0] = vre; o[1] = vim; }
         else if (p.out_mode == OUT_RMW) { o[0] += vre; o[1] += vim; }
         else { atomicAdd(o, vre); atomicAdd(o + 1, vim); }
+    }
+}
+
+// Pads a stream of N inputs per (t, f) row to NP = the next multiple of 16 with stored zeros (0x88 = 0 + 0i),
+// for the TMA-fed paths, whose global strides must be multiples of 16 bytes.  HBM-bound copy.
+__global__ void __launch_bounds__(256)
+corr_pad_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, int N, int NP, long long rows)
+{
+    // a block takes 64 consecutive (t, f) rows at a time; a thread builds 4 output bytes from (up to) 4
+    // consecutive input bytes
+    const int words = NP >> 2;
+    for (long long r0 = (long long)blockIdx.x * 64; r0 < rows; r0 += (long long)gridDim.x * 64) {
+        const int nr = (int)min((long long)64, rows - r0);
+        const uint8_t *src0 = in + r0 * N;
+        uint32_t *dst0 = reinterpret_cast<uint32_t *>(out + r0 * NP);
+        for (int i = threadIdx.x; i < nr * words; i += 256) {
+            const int lr = i / words, w = i - lr * words;
+            const uint8_t *src = src0 + (size_t)lr * N;
+            const int n = 4 * w;
+            uint32_t v = 0x88888888u;
+            if (n + 3 < N) {
+                v = (uint32_t)src[n] | ((uint32_t)src[n + 1] << 8) | ((uint32_t)src[n + 2] << 16) | ((uint32_t)src[n + 3] << 24);
+            } else if (n < N) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (n + j < N) v = (v & ~(0xFFu << (8 * j))) | ((uint32_t)src[n + j] << (8 * j));
+            }
+            dst0[i] = v;
+        }
     }
 }
 

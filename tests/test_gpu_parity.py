@@ -94,6 +94,35 @@ def test_imma_small_n(corr, oracle, N):
     assert info["path"] == corr.PATH_IMMA and np.array_equal(auto, w2)
 
 
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 15, 17, 31, 33, 47, 49, 63, 65, 100, 127, 129, 200, 255, 257, 1000])
+def test_n_not_a_multiple_of_16(corr, oracle, N):
+    # the TMA-fed paths read a copy of the stream padded to the next multiple of 16 inputs with stored zeros;
+    # the output keeps the caller's N.  Automatic path, and both tensor-core paths forced where they apply.
+    for F in (1, 3):
+        for T in (1, 33, 257, 1000):
+            packed = workloads.uniform_bytes(N, F, T, seed=N * 7 + F + T)
+            want = oracle.level1(packed)
+            got, info = _run(corr, packed, prefill=-559038737)
+            assert info["path"] == (corr.PATH_IMMA if N <= 64 else corr.PATH_TCGEN05)
+            assert np.array_equal(got, want), (N, F, T, info)
+            both, _ = _run(corr, packed, accumulate_into=got.copy())
+            assert np.array_equal(both, 2 * want), (N, F, T, "accumulate")
+    packed = workloads.uniform_bytes(N, 2, 300, seed=N)
+    got, _ = _run(corr, packed, corr.PATH_TCGEN05)                 # small N through the big-tile path too
+    assert np.array_equal(got, oracle.level1(packed))
+    # an input pointer that is not 16-byte aligned is fine when the stream is copied anyway
+    import torch
+    T, F = 100, 2
+    packed = workloads.uniform_bytes(N, F, T, seed=1)
+    with corr.Plan(N, F, T) as plan:
+        buf = torch.zeros(packed.size + 64, dtype=torch.uint8, device="cuda")
+        dev = buf[3:3 + packed.size].view(T, F, N)
+        dev.copy_(torch.from_numpy(packed))
+        vis = plan.execute(dev)
+        torch.cuda.synchronize()
+        assert np.array_equal(vis.cpu().numpy(), oracle.level1(packed))
+
+
 def test_tcgen05_extreme_values(corr, oracle):
     # all samples -8-8i: largest products (16*-8 = -128 on both operands), Re = 128 T, Im = 0
     N, F, T = 256, 2, 4096
@@ -311,9 +340,9 @@ def test_invalid_arguments(corr):
         with pytest.raises(corr.CorrError):
             corr.corr_plan_create(*bad)
     with pytest.raises(corr.CorrError):
-        corr.corr_plan_create(100, 1, 64, corr.PATH_TCGEN05)   # N % 16 != 0
+        corr.corr_plan_create(65, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N <= 64
     with pytest.raises(corr.CorrError):
-        corr.corr_plan_create(80, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N = 16, 32, 48, 64 only
+        corr.corr_plan_create(80, 1, 64, corr.PATH_IMMA)       # warp-MMA path: N <= 64 only
 
 
 # ------------------------------------------------------------------ the five BASELINE.json configs
