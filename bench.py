@@ -130,7 +130,7 @@ def run_reference(args, cfg):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8",
         "data": "synthetic",
-        "config": {"workload": f"cfg3 N={cfg.N} F={cfg.F} T={cfg.T} (iid quantised Gaussian sigma 2.5)",
+        "config": {"workload": f"{args.config} N={cfg.N} F={cfg.F} T={cfg.T} ({cfg.kind} recipe of workloads/, DESIGN.md section 4)",
                    "sample_per_step": f"N={cfg.N}, F={Fs}, T={Ts}"},
         "cpu_baseline": {"value": value, "unit": "TOPS", "cores": threads, "kind": "oracle",
                          "sample": f"oracle.level1 on N={cfg.N}, F={Fs}, T={Ts} per step"},
@@ -275,7 +275,7 @@ def main():
         "metric": METRIC, "value": value, "unit": "TOPS", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int8", "data": "synthetic",
-        "config": {"workload": f"cfg3 N={N} F={F} T={T} (iid quantised Gaussian sigma 2.5), one batch per GPU",
+        "config": {"workload": f"{args.config} N={N} F={F} T={T} ({cfg.kind} recipe of workloads/, DESIGN.md section 4), one batch per GPU",
                    "l2": f"{NBUF} rotating inputs of {N * F * T / 1e6:.0f} MB each + {vis.numel() * 4 / 1e6:.0f} MB output per step: larger than the 126 MB L2",
                    "path": plan.info},
         "pct_of_int8_peak": {"nominal_4500": 100 * value / world / NOMINAL_INT8_TOPS,
