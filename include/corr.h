@@ -148,6 +148,18 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
  * This is the ceiling the roofline of section 8(d) is also reported against.  Returns CORR_OK or an error. */
 int corr_measure_int8_tops(int iters, double *tops_out);
 
+/* corr_submit_host / corr_wait_host -- corr_execute_host split in two, for streaming use: submit enqueues the
+ * copies and kernels of one call and returns without waiting for the device, so the copy-in of the next call
+ * overlaps the kernels and the copy-out of this one; corr_wait_host blocks until everything submitted on the
+ * plan so far has finished (results of ALL submitted calls are then in their vis_host buffers).  Between
+ * submit and wait the host buffers of that call must stay valid and untouched; use pinned memory, and a
+ * different vis_host per call in flight unless the calls are meant to accumulate into one buffer
+ * (accumulate_flag != 0 reads vis_host after the previous call's copy-out to it has finished).  All calls
+ * of a plan go on one stream.  corr_execute_host = corr_submit_host + corr_wait_host. */
+int corr_submit_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_host,
+                     int accumulate_flag, corr_stream_t stream);
+int corr_wait_host(corr_plan *plan);
+
 /* corr_plan_destroy -- free the plan and its device scratch.  NULL is a no-op. */
 void corr_plan_destroy(corr_plan *plan);
 

@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops", "corr_submit_host", "corr_wait_host")
 
 
 class CorrError(RuntimeError):
@@ -43,6 +43,10 @@ def load_library():
         lib.corr_execute.restype = ci
         lib.corr_execute_host.argtypes = [vp, vp, vp, ci, vp]
         lib.corr_execute_host.restype = ci
+        lib.corr_submit_host.argtypes = [vp, vp, vp, ci, vp]
+        lib.corr_submit_host.restype = ci
+        lib.corr_wait_host.argtypes = [vp]
+        lib.corr_wait_host.restype = ci
         lib.corr_plan_destroy.argtypes = [vp]
         lib.corr_plan_destroy.restype = None
         lib.corr_last_error.argtypes = []
@@ -129,6 +133,18 @@ def time_shift(packed, lags, out=None, stream=None):
     s = torch.cuda.current_stream(packed.device) if stream is None else stream
     corr_time_shift(N, F, T, packed.data_ptr(), lags.data_ptr(), out.data_ptr(), s.cuda_stream)
     return out
+
+
+def corr_submit_host(plan: int, packed_host_ptr: int, vis_host_ptr: int, accumulate_flag: int, stream: int) -> None:
+    rc = load_library().corr_submit_host(plan, packed_host_ptr, vis_host_ptr, int(bool(accumulate_flag)), stream)
+    if rc != 0:
+        raise CorrError(f"corr_submit_host -> {rc}: {_err()}")
+
+
+def corr_wait_host(plan: int) -> None:
+    rc = load_library().corr_wait_host(plan)
+    if rc != 0:
+        raise CorrError(f"corr_wait_host -> {rc}: {_err()}")
 
 
 def corr_plan_destroy(plan: int) -> None:
@@ -218,6 +234,20 @@ class Plan:
 
         corr_execute_host(self._h, ptr(packed_host), ptr(vis_host), int(accumulate), s.cuda_stream)
         return vis_host
+
+    def submit_host(self, packed_host, vis_host, accumulate: bool = False, stream=None):
+        """execute_host without the final wait: keep both buffers alive and untouched until wait_host()."""
+        import torch
+        s = torch.cuda.current_stream() if stream is None else stream
+
+        def ptr(a):
+            return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+
+        corr_submit_host(self._h, ptr(packed_host), ptr(vis_host), int(accumulate), s.cuda_stream)
+        return vis_host
+
+    def wait_host(self):
+        corr_wait_host(self._h)
 
     def close(self):
         if getattr(self, "_h", None):

@@ -113,7 +113,9 @@ struct corr_plan {
     corr_plan *sub;        // plan for host_fg channels, executed once per group
     int host_fg;           // channels per group (divides F); 0 = not pipelined
     cudaStream_t s_in, s_out;
-    cudaEvent_t ev_start, ev_in[2], ev_free[2], ev_comp, ev_done;
+    cudaEvent_t ev_start, ev_in[2], ev_free[2], ev_out[8], ev_comp, ev_done;
+    unsigned long long grp_seq;   // channel groups submitted so far (staging buffers alternate across calls)
+    unsigned long long calls_submitted;
     // corr_execute_gated: per-gate runs of the gathered stream, plans for their lengths
     uint8_t *gate_buf;     // device, T*F*N bytes: rows regrouped by gate
     int *order_dev;        // device, T row indices
@@ -163,6 +165,7 @@ void corr_plan_destroy(corr_plan *p)
     if (p->tiles4_dev) cudaFree(p->tiles4_dev);
     if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->flags_dev) cudaFree(p->flags_dev);
+    if (p->host_fg != 0) cudaEventDestroy(p->ev_done);
     if (p->gate_plans) {
         for (auto &kv : *p->gate_plans) corr_plan_destroy(kv.second);
         delete p->gate_plans;
@@ -179,7 +182,7 @@ void corr_plan_destroy(corr_plan *p)
         cudaStreamDestroy(p->s_out);
         cudaEventDestroy(p->ev_start);
         cudaEventDestroy(p->ev_comp);
-        cudaEventDestroy(p->ev_done);
+        for (int i = 0; i < 8; ++i) cudaEventDestroy(p->ev_out[i]);
         for (int i = 0; i < 2; ++i) {
             cudaEventDestroy(p->ev_in[i]);
             cudaEventDestroy(p->ev_free[i]);
@@ -768,11 +771,11 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
     return CORR_OK;
 }
 
-int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_host, int accumulate_flag,
-                      corr_stream_t stream_)
+int corr_submit_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_host, int accumulate_flag,
+                     corr_stream_t stream_)
 {
     if (!p || !packed_host || !vis_host) {
-        set_err("corr_execute_host: NULL plan or buffer");
+        set_err("corr_submit_host: NULL plan or buffer");
         return CORR_ERR_INVALID_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -780,32 +783,39 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
 
     // Large transfers: pipeline over groups of channels (channels are independent), so that the
     // host->device copy of group g+1, the kernels of group g and the device->host copy of group g-1 overlap
-    // (PCIe is full duplex).  Each group's slice of the stream is gathered by a strided 2-D copy into a
-    // contiguous [T][Fg][N] staging buffer (two of them, used alternately); its output is contiguous in vis.
-    if (p->host_fg == 0 && !p->sub) {
+    // (PCIe is full duplex) -- inside one call and, because nothing here waits for the device, across
+    // successive calls.  Each group's slice of the stream is gathered by a strided 2-D copy into a contiguous
+    // [T][Fg][N] staging buffer (two of them, used alternately); its output is contiguous in vis.
+    if (p->host_fg == 0) {
         p->host_fg = -1;   // decided once
+        bool ok = cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) == cudaSuccess;
         int groups = 0;
         for (int g = std::min(p->F, 8); g >= 2; --g)
             if (p->F % g == 0) { groups = g; break; }
-        if (groups >= 2 && in_bytes + out_bytes >= (size_t)(32 << 20)) {
+        if (ok && groups >= 2 && in_bytes + out_bytes >= (size_t)(32 << 20)) {
             corr_plan *sub = corr_plan_create_ex(p->N, p->F / groups, p->T, p->path);
             if (sub) {
-                bool ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
-                          cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess;
+                ok = cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+                     cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking) == cudaSuccess;
                 ok = ok && cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming) == cudaSuccess &&
-                     cudaEventCreateWithFlags(&p->ev_comp, cudaEventDisableTiming) == cudaSuccess &&
-                     cudaEventCreateWithFlags(&p->ev_done, cudaEventDisableTiming) == cudaSuccess;
+                     cudaEventCreateWithFlags(&p->ev_comp, cudaEventDisableTiming) == cudaSuccess;
                 for (int i = 0; i < 2 && ok; ++i)
                     ok = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming) == cudaSuccess &&
                          cudaEventCreateWithFlags(&p->ev_free[i], cudaEventDisableTiming) == cudaSuccess;
-                if (!ok) {
-                    set_err("corr_execute_host: cannot create the copy streams/events: %s", cudaGetErrorString(cudaGetLastError()));
+                for (int i = 0; i < 8 && ok; ++i)
+                    ok = cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming) == cudaSuccess;
+                if (ok) {
+                    p->sub = sub;
+                    p->host_fg = p->F / groups;
+                } else {
                     corr_plan_destroy(sub);
-                    return CORR_ERR_CUDA;
                 }
-                p->sub = sub;
-                p->host_fg = p->F / groups;
             }
+        }
+        if (!ok) {
+            set_err("corr_submit_host: cannot create the copy streams/events: %s", cudaGetErrorString(cudaGetLastError()));
+            p->host_fg = 0;
+            return CORR_ERR_CUDA;
         }
     }
     if (p->sub) {
@@ -817,13 +827,19 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
         CUDA_TRY(cudaEventRecord(p->ev_start, stream), CORR_ERR_CUDA);       // everything follows the caller's stream
         CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_start, 0), CORR_ERR_CUDA);
         CUDA_TRY(cudaStreamWaitEvent(p->s_out, p->ev_start, 0), CORR_ERR_CUDA);
-        for (int g = 0; g < groups; ++g) {
-            const int b = g & 1;
+        for (int g = 0; g < groups; ++g, ++p->grp_seq) {
+            const int b = (int)(p->grp_seq & 1);
             uint8_t *din = p->packed_own + (size_t)b * grp_in;
             int32_t *dvis = p->vis_own + (size_t)g * grp_out;
-            if (g >= 2) CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_free[b], 0), CORR_ERR_CUDA);   // staging buffer b is free again
+            if (p->grp_seq >= 2) CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_free[b], 0), CORR_ERR_CUDA);   // staging buffer b is free again
             CUDA_TRY(cudaMemcpy2DAsync(din, (size_t)fg * p->N, packed_host + (size_t)g * fg * p->N, (size_t)p->F * p->N,
                                        (size_t)fg * p->N, (size_t)p->T, cudaMemcpyHostToDevice, p->s_in), CORR_ERR_CUDA);
+            if (p->calls_submitted > 0) {
+                // the previous call's copy-out of this group's image has finished (device image and, when the caller
+                // chains calls through one host buffer, the host data this call reads back in)
+                CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_out[g], 0), CORR_ERR_CUDA);
+                CUDA_TRY(cudaStreamWaitEvent(stream, p->ev_out[g], 0), CORR_ERR_CUDA);
+            }
             if (accumulate_flag)
                 CUDA_TRY(cudaMemcpyAsync(dvis, vis_host + (size_t)g * grp_out, grp_out * sizeof(int32_t),
                                          cudaMemcpyHostToDevice, p->s_in), CORR_ERR_CUDA);
@@ -836,10 +852,10 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
             CUDA_TRY(cudaStreamWaitEvent(p->s_out, p->ev_comp, 0), CORR_ERR_CUDA);
             CUDA_TRY(cudaMemcpyAsync(vis_host + (size_t)g * grp_out, dvis, grp_out * sizeof(int32_t),
                                      cudaMemcpyDeviceToHost, p->s_out), CORR_ERR_CUDA);
+            CUDA_TRY(cudaEventRecord(p->ev_out[g], p->s_out), CORR_ERR_CUDA);
         }
         CUDA_TRY(cudaEventRecord(p->ev_done, p->s_out), CORR_ERR_CUDA);
-        CUDA_TRY(cudaStreamWaitEvent(stream, p->ev_done, 0), CORR_ERR_CUDA);
-        CUDA_TRY(cudaStreamSynchronize(stream), CORR_ERR_CUDA);
+        ++p->calls_submitted;
         return CORR_OK;
     }
     if (!p->packed_own) CUDA_TRY(cudaMalloc(&p->packed_own, in_bytes), CORR_ERR_ALLOC);
@@ -850,8 +866,28 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
     int rc = corr_execute(p, p->packed_own, p->vis_own, accumulate_flag, stream_);
     if (rc != CORR_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(vis_host, p->vis_own, out_bytes, cudaMemcpyDeviceToHost, stream), CORR_ERR_CUDA);
-    CUDA_TRY(cudaStreamSynchronize(stream), CORR_ERR_CUDA);
+    CUDA_TRY(cudaEventRecord(p->ev_done, stream), CORR_ERR_CUDA);
+    ++p->calls_submitted;
     return CORR_OK;
+}
+
+int corr_wait_host(corr_plan *p)
+{
+    if (!p) {
+        set_err("corr_wait_host: NULL plan");
+        return CORR_ERR_INVALID_ARG;
+    }
+    if (p->calls_submitted == 0) return CORR_OK;
+    CUDA_TRY(cudaEventSynchronize(p->ev_done), CORR_ERR_CUDA);   // the last copy-out of the last submitted call
+    return CORR_OK;
+}
+
+int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_host, int accumulate_flag,
+                      corr_stream_t stream_)
+{
+    int rc = corr_submit_host(p, packed_host, vis_host, accumulate_flag, stream_);
+    if (rc != CORR_OK) return rc;
+    return corr_wait_host(p);
 }
 
 }  // extern "C"

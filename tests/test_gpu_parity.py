@@ -286,6 +286,30 @@ def test_execute_host_pipelined(corr, oracle):
         assert np.array_equal(pageable, want)
 
 
+@pytest.mark.parametrize("shape", [(1024, 6, 5500), (160, 2, 700)])   # pipelined over channel groups / small single-stream path
+def test_submit_host_streaming(corr, oracle, shape):
+    # several calls in flight: distinct inputs and outputs, then an accumulating chain through one host buffer
+    import torch
+    N, F, T = shape
+    ins = [workloads.iid_gaussian(N, F, T, seed=30 + k) for k in range(3)]
+    wants = [oracle.level1(a) for a in ins]
+    with corr.Plan(N, F, T) as plan:
+        ph = [torch.from_numpy(a).pin_memory() for a in ins]
+        vh = [torch.full((F, plan.baselines, 2), -1, dtype=torch.int32).pin_memory() for _ in ins]
+        for k in range(3):
+            plan.submit_host(ph[k], vh[k])
+        plan.wait_host()
+        for k in range(3):
+            assert np.array_equal(vh[k].numpy(), wants[k]), (shape, k)
+        acc = torch.zeros((F, plan.baselines, 2), dtype=torch.int32).pin_memory()
+        for k in range(3):
+            plan.submit_host(ph[k], acc, accumulate=True)
+        plan.wait_host()
+        assert np.array_equal(acc.numpy(), wants[0] + wants[1] + wants[2]), shape
+        plan.execute_host(ph[0], acc)                    # the blocking call still works after streaming ones
+        assert np.array_equal(acc.numpy(), wants[0])
+
+
 def test_int32_headroom_edge(corr):
     # pin P10: the largest T the ABI takes, every sample -8-8i: Re = 128 * (2^24 - 1) =
     # 2 147 483 520 on every baseline, Im = 0, no wrap (closed form, PAPER.md:41-44 with constant input)
