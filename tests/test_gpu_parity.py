@@ -308,6 +308,14 @@ def test_submit_host_streaming(corr, oracle, shape):
         assert np.array_equal(acc.numpy(), wants[0] + wants[1] + wants[2]), shape
         plan.execute_host(ph[0], acc)                    # the blocking call still works after streaming ones
         assert np.array_equal(acc.numpy(), wants[0])
+        plan.submit_host(ph[1], acc, accumulate=True)    # ... and the two forms chain through one host buffer
+        plan.execute_host(ph[2], acc, accumulate=True)
+        assert np.array_equal(acc.numpy(), wants[0] + wants[1] + wants[2])
+        for k in range(5):                               # more calls in flight than device images
+            plan.submit_host(ph[k % 3], vh[k % 3])
+        plan.wait_host()
+        for k in range(3):
+            assert np.array_equal(vh[k].numpy(), wants[k]), (shape, k, "second round")
 
 
 def test_int32_headroom_edge(corr):
