@@ -22,12 +22,46 @@ SHAPES = [
 ]
 
 
+def other_op(args):
+    """Times corr_time_shift or corr_execute_gated on one shape (read + written bytes per second for the shift)."""
+    import numpy as np
+    import torch
+    from . import Plan, time_shift
+    n, f, t = (int(v) for v in (args.shape or "2048,8,8192").split(","))
+    dev = torch.device("cuda:0")
+    a = torch.randint(0, 256, (t, f, n), dtype=torch.uint8, device=dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if args.op == "shift":
+        lags = torch.randint(-16, 17, (n,), dtype=torch.int32, device=dev)
+        out = torch.empty_like(a)
+        run = lambda: time_shift(a, lags, out=out)
+    else:
+        plan = Plan(n, f, t)
+        gate = ((np.arange(t) % 64) * 4 // 64).astype(np.int32)
+        vis = plan.execute_gated(a, gate, 4)
+        run = lambda: plan.execute_gated(a, gate, 4, vis=vis)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.reps):
+        run()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.reps
+    print(f"{args.op},N={n},F={f},T={t},ms={ms:.4g},stream_GBs={a.numel() / (ms * 1e-3) / 1e9:.4g}")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--csv", default=None)
     ap.add_argument("--shape", default=None, help="N,F,T: time this one shape only (e.g. under ncu)")
+    ap.add_argument("--op", default="corr", choices=["corr", "shift", "gated"],
+                    help="with --shape: corr_execute (default), corr_time_shift (lags of +-16) or corr_execute_gated (4 gates)")
     args = ap.parse_args()
+    if args.op != "corr":
+        return other_op(args)
     shapes = SHAPES
     if args.shape:
         n, f, t = (int(v) for v in args.shape.split(","))
