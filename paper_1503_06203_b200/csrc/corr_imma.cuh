@@ -243,26 +243,39 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
 __global__ void __launch_bounds__(256)
 corr_pad_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, int N, int NP, long long rows)
 {
-    // a block takes 64 consecutive (t, f) rows at a time; a thread builds 4 output bytes from (up to) 4
-    // consecutive input bytes
-    const int words = NP >> 2;
+    // a block takes 64 consecutive (t, f) rows at a time; a thread builds 16 output bytes from 16 consecutive
+    // input bytes at any alignment (five aligned 32-bit loads and four funnel shifts), or byte by byte at the
+    // end of a row and in the last row of the stream (where reading past the 16 bytes could leave the buffer)
+    const int chunks = NP >> 4;
     for (long long r0 = (long long)blockIdx.x * 64; r0 < rows; r0 += (long long)gridDim.x * 64) {
         const int nr = (int)min((long long)64, rows - r0);
-        const uint8_t *src0 = in + r0 * N;
-        uint32_t *dst0 = reinterpret_cast<uint32_t *>(out + r0 * NP);
-        for (int i = threadIdx.x; i < nr * words; i += 256) {
-            const int lr = i / words, w = i - lr * words;
-            const uint8_t *src = src0 + (size_t)lr * N;
-            const int n = 4 * w;
-            uint32_t v = 0x88888888u;
-            if (n + 3 < N) {
-                v = (uint32_t)src[n] | ((uint32_t)src[n + 1] << 8) | ((uint32_t)src[n + 2] << 16) | ((uint32_t)src[n + 3] << 24);
-            } else if (n < N) {
+        for (int i = threadIdx.x; i < nr * chunks; i += 256) {
+            const int lr = i / chunks, c = i - lr * chunks;
+            const long long r = r0 + lr;
+            const uint8_t *src = in + r * N + 16 * c;
+            uint32_t v[4];
+            if (16 * c + 16 <= N && r + 1 < rows) {
+                const uintptr_t a = reinterpret_cast<uintptr_t>(src);
+                const uint32_t *al = reinterpret_cast<const uint32_t *>(a & ~(uintptr_t)3);
+                const uint32_t sh = 8u * (uint32_t)(a & 3);
+                uint32_t w[5];
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (n + j < N) v = (v & ~(0xFFu << (8 * j))) | ((uint32_t)src[n + j] << (8 * j));
+                for (int k = 0; k < 5; ++k) w[k] = __ldg(al + k);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) v[k] = __funnelshift_r(w[k], w[k + 1], sh);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    uint32_t x = 0;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int n = 16 * c + 4 * k + j;
+                        x |= (uint32_t)((n < N) ? src[4 * k + j] : (uint8_t)0x88) << (8 * j);
+                    }
+                    v[k] = x;
+                }
             }
-            dst0[i] = v;
+            *reinterpret_cast<uint4 *>(out + r * NP + 16 * c) = make_uint4(v[0], v[1], v[2], v[3]);
         }
     }
 }
