@@ -4,8 +4,9 @@
 // Why not dp4a here: measured on B200, IDP.4A issues 64 lanes/clk/SM = 17.5 T dp4a/s, i.e. 140
 // effective TOPS at one dp4a per complex MAC, while streaming N = 16 inputs at HBM speed needs
 // 4 (N + 1) ops per byte x 6.5 TB/s = 440 effective TOPS.  The legacy warp-level IMMA path
-// measures 1146 TOPS, enough to stay memory-bound up to N = 32 (corr_dp4a.cuh remains the path
-// for every other small N).  The paper makes the small-N observation for its own tiles at
+// measures 1146 TOPS, enough to stay memory-bound up to N = 32.  Other N <= 64 run here on a stream
+// padded to the next multiple of 16 inputs (corr_pad_kernel below); corr_dp4a.cuh is only used on
+// request.  The paper makes the small-N observation for its own tiles at
 // PAPER.md:72; the result computed is Eq. 1 summed over time on the
 // upper triangle.
 //
