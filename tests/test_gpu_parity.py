@@ -367,6 +367,13 @@ def test_no_write_outside_the_output(corr, oracle, case):
             os.environ.pop("CORR_TC_VARIANT", None)
 
 
+def test_int8_issue_loop_measurement(corr):
+    # measurement aid: a bare tcgen05.mma.kind::i8 issue loop; on a B200 it lands between the power-capped and the
+    # boost-clock ceiling (8192 MAC/clk/SM x 148 SMs x 2 ops at 1.3 .. 1.97 GHz)
+    tops = corr.corr_measure_int8_tops(5000)
+    assert 2500.0 < tops < 5000.0, tops
+
+
 def test_invalid_arguments(corr):
     for bad in [(0, 1, 1), (16, 0, 1), (16, 1, 0), (16, 1, 1 << 24)]:
         with pytest.raises(corr.CorrError):
