@@ -31,10 +31,49 @@ if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
 METRIC = "effective correlation TOPS (8 ops/CMAC/baseline) at N=2048; % of int8 TC peak"
-# dram__bytes_read.sum + dram__bytes_write.sum of one corr_tc3_kernel launch on cfg3, from the ncu --set full
-# capture summarised in profiles/r01_tc3_ncu_summary.md (136.4 MB + 98.7 MB; algorithmic: 134.2 + 134.3 MB)
-NCU_DRAM_BYTES_PER_LAUNCH = 235.1e6
 NOMINAL_INT8_TOPS = 4500.0  # dense int8 = 2x dense bf16 2250 (B200_PROFILING.md nominal table)
+# roofline.traffic comes from a tracked ncu summary (profiles/), which records the kernel it was captured on and
+# the SHA-256 of that kernel's sources at capture time; a stale record (sources changed since) reports null.
+TRAFFIC_RECORD = ROOT / "profiles" / "tc_traffic.txt"
+KERNEL_SOURCES = ("corr_tc3.cuh", "corr_tc4.cuh", "corr_ptx.cuh", "corr_api.cu")
+
+# the N sweep of the paper's Fig. 4 axis (inputs >= 256 MB for small N so that GB/s means something)
+# and the five BASELINE.json shapes: (label, N, F, T, accumulate)
+TABLE_SHAPES = [
+    ("n16", 16, 256, 65536, 0), ("n32", 32, 128, 65536, 0), ("n64", 64, 64, 65536, 0), ("n128", 128, 64, 32768, 0),
+    ("n256", 256, 32, 32768, 0), ("n512", 512, 32, 16384, 0), ("n1024", 1024, 16, 16384, 0),
+    ("n2048", 2048, 8, 16384, 0), ("n4096", 4096, 4, 8192, 0), ("n8192", 8192, 1, 8192, 0),
+    ("cfg1", 16, 4, 1024, 0), ("cfg2", 256, 16, 16384, 0), ("cfg3", 2048, 8, 8192, 0), ("cfg4", 8192, 1, 4096, 0),
+    ("cfg5_one_accumulate_call", 512, 64, 8192, 1),
+]
+
+
+def kernel_source_sha():
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update((ROOT / "paper_1503_06203_b200" / "csrc" / name).read_bytes())
+    return h.hexdigest()
+
+
+def recorded_traffic(kernel: str, workload: str):
+    """dram bytes (read + write) per launch from profiles/tc_traffic.txt, or None if there is no record for this
+    kernel and workload or the kernel sources have changed since the capture."""
+    if not TRAFFIC_RECORD.exists():
+        return None, "no record"
+    rec = {}
+    for ln in TRAFFIC_RECORD.read_text().splitlines():
+        if "=" in ln and not ln.lstrip().startswith("#"):
+            k, v = ln.split("=", 1)
+            rec[k.strip()] = v.strip()
+    if rec.get("kernel") != kernel or rec.get("workload") != workload:
+        return None, "record is for another kernel/workload"
+    if rec.get("source_sha256") != kernel_source_sha():
+        return None, f"stale: kernel sources changed since the capture at commit {rec.get('commit', '?')}"
+    try:
+        return float(rec["dram_bytes_read"]) + float(rec["dram_bytes_write"]), f"ncu capture at commit {rec.get('commit', '?')}"
+    except (KeyError, ValueError):
+        return None, "malformed record"
 
 
 def eff_ops(N: int, F: int, T: int) -> float:
@@ -110,6 +149,46 @@ def oracle_sample_tops(N, F, T, seed):
     return eff_ops(N, F, T) / dt / 1e12, dt, oracle.threads()
 
 
+def config_table(corr, dev, peaks, reps=20):
+    """ms, effective TOPS, GB/s and the fraction of the bounding roofline for every shape of TABLE_SHAPES.
+    Inputs are random bytes made on the device (every byte is a legal sample; timing does not depend on values),
+    two rotating buffers (eight for small inputs) so that successive calls do not find their input in L2."""
+    import torch
+    int8_peak = 2.0 * float(peaks["bf16_tflops"])
+    hbm_peak = float(peaks["hbm_gbs"])
+    out = {}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for label, N, F, T, acc in TABLE_SHAPES:
+        plan = corr.Plan(N, F, T)
+        nbuf = 2 if N * F * T >= (64 << 20) else 8
+        ins = [torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device=dev) for _ in range(nbuf)]
+        vis = torch.zeros((F, plan.baselines, 2), dtype=torch.int32, device=dev)
+        for i in range(3):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        torch.cuda.synchronize(dev)
+        e0.record()
+        for i in range(reps):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        ms = e0.elapsed_time(e1) / reps
+        tops = eff_ops(N, F, T) / (ms * 1e-3) / 1e12
+        gbs = (N * F * T + vis.numel() * 4 * (2 if acc else 1)) / (ms * 1e-3) / 1e9
+        # 4 (N + 1) ops per input byte against the ridge int8_peak / hbm_peak: HBM-bound below it
+        hbm_bound = 4.0 * (N + 1) < int8_peak * 1e12 / (hbm_peak * 1e9)
+        row = {"N": N, "F": F, "T": T, "ms": round(ms, 5), "value": round(tops, 2), "gbs": round(gbs, 1),
+               "path": plan.info["path"], "bound": "hbm" if hbm_bound else "tensor",
+               "frac": round(gbs / hbm_peak if hbm_bound else tops / int8_peak, 4),
+               "frac_of_nominal_4500": round(tops / NOMINAL_INT8_TOPS, 4)}
+        if label == "cfg1":
+            row["bound"] = "launch latency (64 KB of input)"
+        out[label] = row
+        plan.close()
+        del ins, vis
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_reference(args, cfg):
     """The reference arm for this tier is the CPU oracle (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -148,6 +227,9 @@ def main():
     ap.add_argument("--config", default="cfg3", help="workload (BASELINE.json config name)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sustained-seconds", type=float, default=2.5,
+                    help="length of the sustained leg on the same workload (N=1 only; 0 = skip)")
+    ap.add_argument("--no-table", action="store_true", help="skip the per-config / N-sweep table (N=1 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -211,6 +293,28 @@ def main():
     ms_per_step = ms_total / args.steps
     value = eff_ops(N, F, T) * world / (ms_per_step * 1e-3) / 1e12
 
+    # ---- sustained leg: the same step back to back for >= 2 s (the headline above is a burst of a few ms, during
+    #      which the part holds its boost clock; under sustained load it is power-capped)
+    sustained = None
+    if world == 1 and args.sustained_seconds > 0:
+        n_sus = max(args.steps, int(args.sustained_seconds * 1e3 / ms_per_step))
+        sampler_s = ClockSampler(local_rank)
+        torch.cuda.synchronize(dev)
+        sampler_s.start()
+        e0.record(stream)
+        for i in range(n_sus):
+            plan.execute(dev_inputs[i % NBUF], vis)
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        ms_sus = e0.elapsed_time(e1) / n_sus
+        sustained = {"value": eff_ops(N, F, T) / (ms_sus * 1e-3) / 1e12, "unit": "TOPS", "steps": n_sus,
+                     "ms_per_step": ms_sus, "seconds": ms_sus * n_sus * 1e-3, "clocks": sampler_s.stop()}
+
+    # ---- per-config table: the five BASELINE.json shapes and the N sweep, same process, device-timed
+    table = None
+    if world == 1 and not args.no_table:
+        table = config_table(corr, dev, measured_peaks()[0])
+
     # ---- e2e: host buffers through the library's host API, copies inside the timed region.  Streaming use
     #      (corr_submit_host per step, one corr_wait_host at the end): every step copies its 134 MB in from pinned
     #      host memory and its 134 MB result back out; successive steps overlap on the PCIe link.
@@ -253,13 +357,16 @@ def main():
     if path == corr.PATH_TCGEN05:
         variant = os.environ.get("CORR_TC_VARIANT", "3")
         kernel = {"1": "corr_tc_kernel", "2": "corr_tc2_kernel", "4": "corr_tc4_kernel"}.get(variant, "corr_tc3_kernel")
+        traffic, traffic_source = recorded_traffic(kernel, args.config)
         roofline = {
             "bound": "tensor", "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak,
-            "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.config == "cfg3" and kernel == "corr_tc3_kernel") else None,
+            "traffic": traffic, "traffic_source": traffic_source,
             "peak_source": f"2 x bf16_tflops burst of MEASURED_PEAKS.json ({peaks_kind}); int8:bf16 nominal ratio 2",
             "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS,
             "int8_issue_loop_tops": int8_measured, "frac_of_int8_issue_loop": achieved / int8_measured,
-            "frac_of_sustained": achieved / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))),
+            # the sustained leg against the sustained denominator (both power-capped); burst against burst is `frac`
+            "frac_of_sustained": (sustained["value"] / (2.0 * float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])))
+                                  if sustained else None),
             "kernel": kernel, "kernel_ms": kernel_ms,
             "algorithmic_ops_per_launch": eff_ops(N, F, T),
         }
@@ -300,6 +407,8 @@ def main():
                 "blocking_value": eff_ops(N, F, T) * world / e2e_blocking_s / 1e12},
         "gpu_launches": args.steps * plan.info["kernels"],
         "roofline": roofline,
+        "sustained": sustained,
+        "configs": table,
         "cpu_baseline": cpu_baseline,
         "paper_context": "5.6 effective TOPS on a 4.3 TOPS AMD R9 280X (PAPER.md:15); another machine",
     }

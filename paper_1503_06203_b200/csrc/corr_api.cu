@@ -26,6 +26,7 @@
 namespace {
 
 thread_local char g_err[512] = "";
+thread_local int g_create_rc = 0;   // error code of the last failed corr_plan_create_ex in this thread
 
 void set_err(const char *fmt, ...)
 {
@@ -77,6 +78,8 @@ int count_tiles(int N, int tx, int ty)
 
 }  // namespace
 
+static bool alloc_pad_buf(struct corr_plan *p);
+
 struct corr_plan {
     int N, F, T, path;
     int n_pad;         // N rounded up to a multiple of 16: the width of the stream the TMA-fed kernels read
@@ -101,7 +104,6 @@ struct corr_plan {
     int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
     long long total_groups;
     int *flags_dev;    // variant 3: [num_units][2] stream-K flags (corr_tc3.cuh)
-    int epoch;         // corr_execute calls so far
     int32_t *sums_dev; // variant 4: [2][slices][F][N] per-element sums of the stored bytes
     CUtensorMap tmap;
     CUtensorMap tmap_y;
@@ -123,6 +125,23 @@ struct corr_plan {
     cudaEvent_t ev_gate;   // the upload of order_pin has been consumed
     std::map<int, corr_plan *> *gate_plans;   // length of a run -> plan (N, F, length)
 };
+
+extern "C" void corr_plan_destroy(corr_plan *p);
+
+// N % 16 != 0 on a TMA-fed path: the padded copy of the stream lives in the plan from creation on, so that
+// corr_execute only enqueues work (no allocation, no implicit synchronisation, capturable into a CUDA graph).
+static bool alloc_pad_buf(corr_plan *p)
+{
+    if (p->path == CORR_PATH_DP4A || p->n_pad == p->N) return true;
+    if (cudaMalloc(&p->pad_buf, (size_t)p->T * p->F * p->n_pad) != cudaSuccess) {
+        g_create_rc = CORR_ERR_ALLOC;
+        set_err("corr_plan_create: device allocation of the padded stream (%zu bytes) failed: %s",
+                (size_t)p->T * p->F * p->n_pad, cudaGetErrorString(cudaGetLastError()));
+        corr_plan_destroy(p);
+        return false;
+    }
+    return true;
+}
 
 extern "C" {
 
@@ -196,26 +215,26 @@ void corr_plan_destroy(corr_plan *p)
 corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
 {
     if (N < 1 || F < 1 || T < 1 || T > 16777215) {
-        set_err("corr_plan_create: need N >= 1, F >= 1, 1 <= T <= 16777215 (got N=%d F=%d T=%d)", N, F, T);
+        g_create_rc = CORR_ERR_INVALID_ARG; set_err("corr_plan_create: need N >= 1, F >= 1, 1 <= T <= 16777215 (got N=%d F=%d T=%d)", N, F, T);
         return nullptr;
     }
     if (N > 65535 * 16) {
-        set_err("corr_plan_create: N=%d too large for the tile table", N);
+        g_create_rc = CORR_ERR_INVALID_ARG; set_err("corr_plan_create: N=%d too large for the tile table", N);
         return nullptr;
     }
     if (path != CORR_PATH_AUTO && path != CORR_PATH_DP4A && path != CORR_PATH_TCGEN05 && path != CORR_PATH_IMMA) {
-        set_err("corr_plan_create: unknown path %d", path);
+        g_create_rc = CORR_ERR_INVALID_ARG; set_err("corr_plan_create: unknown path %d", path);
         return nullptr;
     }
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
-        set_err("corr_plan_create: no usable CUDA device (%s); this library has no CPU fallback",
+        g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: no usable CUDA device (%s); this library has no CPU fallback",
                 cudaGetErrorString(cudaGetLastError()));
         return nullptr;
     }
     if (prop.major != 10) {
-        set_err("corr_plan_create: device '%s' is sm_%d%d; this library is built for sm_100a only", prop.name,
+        g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: device '%s' is sm_%d%d; this library is built for sm_100a only", prop.name,
                 prop.major, prop.minor);
         return nullptr;
     }
@@ -232,13 +251,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             path = (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;   // both measured 3-10x the dp4a kernel
     }
     if (path == CORR_PATH_IMMA && n_pad > 64) {
-        set_err("corr_plan_create: the warp-MMA path takes N <= 64, got N=%d", N);
+        g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: the warp-MMA path takes N <= 64, got N=%d", N);
         return nullptr;
     }
 
     corr_plan *p = new (std::nothrow) corr_plan();
     if (!p) {
-        set_err("corr_plan_create: out of host memory");
+        g_create_rc = CORR_ERR_ALLOC; set_err("corr_plan_create: out of host memory");
         return nullptr;
     }
     memset(p, 0, sizeof(*p));
@@ -252,7 +271,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     if (path == CORR_PATH_IMMA) {
         // whole channels per CTA: strips of 128/N channels x chunks of time samples (corr_imma.cuh)
         if (!get_encode_fn()) {
-            set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
+            g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
             delete p;
             return nullptr;
         }
@@ -270,20 +289,24 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, corr::corr_imma_kernel<4>, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES);
         }
         if (e != cudaSuccess || occ < 1) {
-            set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::IM_SMEM_BYTES, cudaGetErrorString(e));
+            g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cannot reserve %d B of shared memory: %s", corr::IM_SMEM_BYTES, cudaGetErrorString(e));
             delete p;
             return nullptr;
         }
         // time chunks (>= 512 samples each): the count that fills whole waves of CTA slots best
+        // int32 headroom: a chunk accumulates 256 * sum (x16 planes) in registers and in the shared-memory
+        // reduction, |256 * 128 * chunk| < 2^31 needs chunk <= 65535; IM_MAX_CHUNK = 32768 leaves a factor 2
         const int slots = p->sm_count * occ;
-        int chunks = 1;
+        const int min_chunks = (T + corr::IM_MAX_CHUNK - 1) / corr::IM_MAX_CHUNK;
+        int chunks = min_chunks;
         double best = 0.0;
-        for (int c = 1; c <= std::max(1, std::min(T / 512, 4 * slots / strips + 1)); ++c) {
+        for (int c = min_chunks; c <= std::max(min_chunks, std::min(T / 512, 4 * slots / strips + 1)); ++c) {
             const long long units = (long long)strips * c;
             const double eff = (double)units / (double)(((units + slots - 1) / slots) * slots);
             if (eff > best + 0.10) { best = eff; chunks = c; }   // more chunks only for a clearly better fill
         }
-        if (const char *cc = getenv("CORR_IMMA_CHUNKS")) chunks = std::max(1, std::min(atoi(cc), std::max(1, T / 128)));  // testing aid
+        if (const char *cc = getenv("CORR_IMMA_CHUNKS"))   // testing aid
+            chunks = std::max(min_chunks, std::min(atoi(cc), std::max(1, T / 128)));
         p->t_per_slice = ((T + chunks - 1) / chunks + corr::IM_ROWS - 1) / corr::IM_ROWS * corr::IM_ROWS;
         p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
         p->tile = N;
@@ -291,6 +314,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->num_units = strips * p->slices;
         p->grid = p->num_units;
         p->kernels_per_exec = (n_pad != N) ? 2 : 1;
+        if (!alloc_pad_buf(p)) return nullptr;
         return p;
     }
 
@@ -304,7 +328,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         const char *v = getenv("CORR_TC_VARIANT");
         p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : (v && !strcmp(v, "4")) ? 4 : 3;
         if (p->variant != 3 && n_pad != N) {
-            set_err("corr_plan_create: CORR_TC_VARIANT=%d needs N %% 16 == 0 (only the default kernel reads a padded stream), got N=%d",
+            g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: CORR_TC_VARIANT=%d needs N %% 16 == 0 (only the default kernel reads a padded stream), got N=%d",
                     p->variant, N);
             delete p;
             return nullptr;
@@ -342,7 +366,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->tiles_per_f = (int)tiles.size();
     const long long units0 = (long long)F * p->tiles_per_f;
     if (units0 > 0x7fffffffLL / 64) {
-        set_err("corr_plan_create: too many work units");
+        g_create_rc = CORR_ERR_INVALID_ARG; set_err("corr_plan_create: too many work units");
         delete p;
         return nullptr;
     }
@@ -387,7 +411,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->grid = 2 * (int)std::min<long long>(p->total_groups, p->sm_count / 2);
         if (cudaMalloc(&p->flags_dev, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess ||
             cudaMemset(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess) {
-            set_err("corr_plan_create: device allocation of the schedule flags failed: %s",
+            g_create_rc = CORR_ERR_ALLOC; set_err("corr_plan_create: device allocation of the schedule flags failed: %s",
                     cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
             return nullptr;
@@ -399,14 +423,14 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         (!tiles4.empty() &&
          (cudaMalloc(&p->tiles4_dev, tiles4.size() * sizeof(ushort4)) != cudaSuccess ||
           cudaMemcpy(p->tiles4_dev, tiles4.data(), tiles4.size() * sizeof(ushort4), cudaMemcpyHostToDevice) != cudaSuccess))) {
-        set_err("corr_plan_create: device allocation of the tile table failed: %s",
+        g_create_rc = CORR_ERR_ALLOC; set_err("corr_plan_create: device allocation of the tile table failed: %s",
                 cudaGetErrorString(cudaGetLastError()));
         corr_plan_destroy(p);
         return nullptr;
     }
     if (path == CORR_PATH_TCGEN05) {
         if (!get_encode_fn()) {
-            set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
+            g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cuTensorMapEncodeTiled not available from the driver");
             corr_plan_destroy(p);
             return nullptr;
         }
@@ -422,12 +446,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (e3 == cudaSuccess && p->variant == 4)
             e3 = cudaMalloc(&p->sums_dev, 2 * (size_t)p->slices * F * N * sizeof(int32_t));
         if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
-            set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
+            g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
                     corr::T2_SMEM_BYTES, corr::T3_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
             return nullptr;
         }
     }
+    if (!alloc_pad_buf(p)) return nullptr;
     return p;
 }
 
@@ -482,12 +507,9 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
         set_err("corr_time_shift: buffers must be 16-byte aligned");
         return CORR_ERR_INVALID_ARG;
     }
-    static bool attr_set = false;
-    if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(corr::corr_shift_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::SH_SMEM_BYTES),
-                 CORR_ERR_CUDA);
-        attr_set = true;
-    }
+    // the attribute belongs to the current device's context: set it on every call (a host-side table write)
+    CUDA_TRY(cudaFuncSetAttribute(corr::corr_shift_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::SH_SMEM_BYTES),
+             CORR_ERR_CUDA);
     dim3 grid((unsigned)((N + 127) / 128), (unsigned)F, (unsigned)((T + corr::SH_TB - 1) / corr::SH_TB));
     corr::corr_shift_kernel<<<grid, corr::SH_THREADS, corr::SH_SMEM_BYTES, static_cast<cudaStream_t>(stream_)>>>(
         packed_in_dev, packed_out_dev, lags_dev, N, F, T);
@@ -553,7 +575,6 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     if (padded) {
         // N % 16 != 0: the TMA-fed kernels read a copy of the stream padded to n_pad inputs with stored zeros
         const long long rows = (long long)p->T * p->F;
-        if (!p->pad_buf) CUDA_TRY(cudaMalloc(&p->pad_buf, (size_t)rows * p->n_pad), CORR_ERR_ALLOC);
         corr::corr_pad_kernel<<<8 * p->sm_count, 256, 0, stream>>>(packed_dev, p->pad_buf, p->N, p->n_pad, rows);
         CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
         packed_dev = p->pad_buf;
@@ -641,11 +662,6 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.groups_full = p->groups_full;
             prm.groups_last = p->groups_last;
             prm.total_groups = p->total_groups;
-            if (p->epoch == 0x7fffffff) {   // the call counter wraps: forget every flag of the previous era
-                CUDA_TRY(cudaMemsetAsync(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int), stream), CORR_ERR_CUDA);
-                p->epoch = 0;
-            }
-            prm.epoch = ++p->epoch;
             prm.flags = p->flags_dev;
             prm.tiles = p->tiles4_dev;
             prm.vis = vis_dev;
@@ -703,12 +719,33 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
         }
         if (g >= 0) ++count[(size_t)g];
     }
+    if (row_bytes % 16 == 0 && (reinterpret_cast<uintptr_t>(packed_dev) & 15u)) {
+        set_err("corr_execute_gated: packed_dev must be 16-byte aligned");
+        return CORR_ERR_INVALID_ARG;
+    }
     if (!p->order_pin) {
-        CUDA_TRY(cudaMallocHost(&p->order_pin, (size_t)T * sizeof(int)), CORR_ERR_ALLOC);
-        CUDA_TRY(cudaEventCreateWithFlags(&p->ev_gate, cudaEventDisableTiming), CORR_ERR_CUDA);
-        CUDA_TRY(cudaMalloc(&p->order_dev, (size_t)T * sizeof(int)), CORR_ERR_ALLOC);
-        CUDA_TRY(cudaMalloc(&p->gate_buf, (size_t)T * row_bytes + 16 * (size_t)T + 16), CORR_ERR_ALLOC);   // + alignment padding per run
-        p->gate_plans = new std::map<int, corr_plan *>();
+        // first gated call of the plan: all of the scratch or none of it (order_pin is the "ready" mark, set last)
+        int *pin = nullptr, *odev = nullptr;
+        uint8_t *gbuf = nullptr;
+        cudaEvent_t ev = nullptr;
+        const bool ok = cudaMallocHost(&pin, (size_t)T * sizeof(int)) == cudaSuccess &&
+                        cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess &&
+                        cudaMalloc(&odev, (size_t)T * sizeof(int)) == cudaSuccess &&
+                        cudaMalloc(&gbuf, (size_t)T * row_bytes + 16 * (size_t)T + 16) == cudaSuccess;   // + alignment padding per run
+        std::map<int, corr_plan *> *plans = ok ? new (std::nothrow) std::map<int, corr_plan *>() : nullptr;
+        if (!ok || !plans) {
+            set_err("corr_execute_gated: allocation of the gating scratch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            if (gbuf) cudaFree(gbuf);
+            if (odev) cudaFree(odev);
+            if (ev) cudaEventDestroy(ev);
+            if (pin) cudaFreeHost(pin);
+            return CORR_ERR_ALLOC;
+        }
+        p->ev_gate = ev;
+        p->order_dev = odev;
+        p->gate_buf = gbuf;
+        p->gate_plans = plans;
+        p->order_pin = pin;
     } else {
         CUDA_TRY(cudaEventSynchronize(p->ev_gate), CORR_ERR_CUDA);   // the previous call's upload has left order_pin
     }
@@ -757,12 +794,18 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
         }
         auto it = p->gate_plans->find(len);
         if (it == p->gate_plans->end()) {
-            if (p->gate_plans->size() >= 64) {   // bound the cache (cudaFree in destroy waits for the device)
-                for (auto &kv : *p->gate_plans) corr_plan_destroy(kv.second);
-                p->gate_plans->clear();
+            if (p->gate_plans->size() >= 64) {
+                // bound the cache: drop ONE plan whose run length this call does not use (its kernels, if any are
+                // still in flight from an earlier call, are waited for by the cudaFree inside destroy)
+                for (auto ev = p->gate_plans->begin(); ev != p->gate_plans->end(); ++ev)
+                    if (std::find(count.begin(), count.end(), ev->first) == count.end()) {
+                        corr_plan_destroy(ev->second);
+                        p->gate_plans->erase(ev);
+                        break;
+                    }
             }
             corr_plan *np = corr_plan_create_ex(p->N, p->F, len, p->path);
-            if (!np) return CORR_ERR_ALLOC;
+            if (!np) return g_create_rc;   // the sub-plan's own error (message already set)
             it = p->gate_plans->emplace(len, np).first;
         }
         int rc = corr_execute(it->second, p->gate_buf + off[(size_t)g], vis_g, accumulate_flag, stream_);

@@ -39,6 +39,7 @@ namespace corr {
 constexpr int IM_ROWS = 128;                 // time samples per stage
 constexpr int IM_STAGE_BYTES = IM_ROWS * 128;
 constexpr int IM_STAGES = 6;
+constexpr int IM_MAX_CHUNK = 32768;          // time samples per CTA: 256 * 128 * chunk stays far below 2^31 (multiple of IM_ROWS)
 constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 256;
 
 template <int NT16> struct ImmaCfg {

@@ -73,8 +73,7 @@ struct Tc3Params {
     int groups_full;   // groups of T3_GROUP samples in a full slice
     int groups_last;   // ... in the last slice of a tile
     long long total_groups;  // over all units
-    int epoch;         // corr_execute call counter of the plan, > 0
-    int *flags;        // [num_units][2]: == epoch once the storing segment of (unit, CTA rank) is in memory;
+    int *flags;        // [num_units][2]: claim / stored state of (unit, CTA rank), see tc3_claim_store;
                        // [2 * num_units]: CTAs that have finished (the last one clears the array for the next launch)
     const ushort4 *tiles;  // (xa, xb, by, flags): 128-blocks of the rows of CTA 0 and CTA 1, of the columns; see Tc3Tile
     int32_t *vis;
@@ -154,6 +153,23 @@ __device__ __forceinline__ bool tc3_next_segment(const Tc3Params &p, Tc3Iter &it
     return true;
 }
 
+// Flag of (unit, CTA rank): 0 = untouched, CLAIMED = one piece is storing, STORED = its store is in memory.
+constexpr int TC3_FLAG_CLAIMED = 1, TC3_FLAG_STORED = 2;
+
+// Called by all epilogue threads of a CTA (warp-uniform control flow).  Returns true in the CTA whose piece
+// stores (the first to arrive); in every other CTA it returns, false, once the store is visible.
+__device__ __forceinline__ bool tc3_claim_store(int *flag, volatile int *claim_smem)
+{
+    if (threadIdx.x == 32 * T3_EPI_WARP0) *claim_smem = atomicCAS(flag, 0, TC3_FLAG_CLAIMED);
+    ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);
+    const int before = *claim_smem;
+    ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);   // everyone has read the slot before its next use
+    if (before == 0) return true;
+    while (ptx::ld_acquire_gpu(flag) != TC3_FLAG_STORED) {
+    }
+    return false;
+}
+
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T3_THREADS, 1)
 corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ CUtensorMap tmap_y,
                 const Tc3Params p)
@@ -174,6 +190,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     const uint32_t acc_empty = acc_full + 8u;
     const uint32_t tmem_slot = acc_empty + 8u;
     volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + (tmem_slot - base));
+    volatile int *claim_g = reinterpret_cast<volatile int *>(gbase + (tmem_slot + 8u - base));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = ptx::cluster_ctarank();  // 0 = leader (issues the MMAs)
@@ -365,13 +382,12 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         uint32_t acc_ph = 0;
         while (tc3_next_segment(p, sit, sg)) {
             // A unit cut by the stream-K schedule is summed in memory.  When the call overwrites (OUT_STORE),
-            // the segment that ends the unit stores and then raises the unit's flag; every other segment of
-            // the unit waits for the flag and adds.  The storing segment is always the FIRST work of its CTA
-            // pair (a pair's range is contiguous), so it never waits on anything: no deadlock.
-            const bool partial = (sg.cnt != sg.len), last = (sg.first + sg.cnt == sg.len);
-            const bool add = base_add || (partial && !last);
-            const bool wait_flag = !base_add && partial && !last;
-            const bool raise_flag = !base_add && partial && last;
+            // the piece that gets to its output FIRST claims the unit (atomic compare-and-swap on the unit's flag),
+            // stores, and then marks the flag "stored"; every later piece waits for that mark and adds.  A waiting
+            // CTA therefore only ever waits for a CTA that is resident and already in its epilogue: no piece
+            // depends on a CTA that has not been scheduled yet, whatever else shares the GPU.
+            const bool claim = !base_add && (sg.cnt != sg.len);   // a piece of a cut unit in a call that overwrites
+            bool add = base_add, raise_flag = false;
             int *flag = p.flags + 2 * sg.u + (int)rank;
             const int f = sg.f;
             const ushort4 tile = sg.tile;
@@ -386,9 +402,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                 ptx::mbar_wait_cluster(acc_full, acc_ph);
                 acc_ph ^= 1u;
                 ptx::tc_fence_after_sync();
-                if (wait_flag)
-                    while (ptx::ld_acquire_gpu(flag) != p.epoch) {
-                    }
+                if (claim) add = !tc3_claim_store(flag, claim_g), raise_flag = !add;
                 const int yt = x;   // true y of this thread
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -453,9 +467,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
             // ---- write the row segment [jlo, jhi) of this thread
             int jlo = max(64 * h, x - y0), jhi = min(64 * h + 64, p.N - y0);
-            if (wait_flag)
-                while (ptx::ld_acquire_gpu(flag) != p.epoch) {
-                }
+            if (claim) add = !tc3_claim_store(flag, claim_g), raise_flag = !add;
             if (x < p.N && jlo < jhi) {
                 ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
                 if ((par + jlo) & 1) {           // leading baseline on an odd 8-byte slot
@@ -481,7 +493,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                 ptx::bulk_wait0();                 // this thread's part of the tile is in memory ...
                 __threadfence();
                 ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);   // ... and so is every other epilogue thread's
-                if (threadIdx.x == 32 * T3_EPI_WARP0) ptx::st_release_gpu(flag, p.epoch);
+                if (threadIdx.x == 32 * T3_EPI_WARP0) ptx::st_release_gpu(flag, TC3_FLAG_STORED);
             }
         }
         ptx::bulk_wait0();  // every row segment has been written before the CTA retires
@@ -491,7 +503,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     ptx::tc_fence_before_sync();
     ptx::cluster_sync();  // no CTA of the pair may exit while its peer still reads its smem / barriers
     if (warp == 1) ptx::tmem_dealloc<2>(tmem, 512);
-    // The last CTA to get here clears the flags, so that a launch replayed with the same call counter (a
+    // The last CTA to get here clears the flags, so that the next launch (or a replay of this one from a
     // captured CUDA graph) starts from a clean array: nobody reads a flag after its own CTA has counted itself.
     if (threadIdx.x == 0) {
         __threadfence();

@@ -337,6 +337,65 @@ def test_int32_headroom_edge(corr):
     assert (got[..., 0] == 128 * T).all() and (got[..., 1] == 0).all()
 
 
+@pytest.mark.parametrize("N,F", [(16, 2368), (32, 592), (48, 296), (64, 296)])
+def test_imma_headroom_when_the_strips_fill_the_gpu(corr, N, F):
+    # The warp-MMA path accumulates 256 * sum (x16 planes) per time chunk, so a chunk must stay below 65536
+    # samples whatever the wave-fill heuristic would like: F is chosen so that ONE chunk per strip already fills
+    # whole waves (148 or 296 CTAs), T = 70000 of the byte 0x00 (-8-8i) would then wrap an int32 accumulator
+    # (256 * 128 * 70000 > 2^31).  Closed form (pin P2): Re = 128 T, Im = 0 on every baseline.
+    import torch
+    T = 70000
+    with corr.Plan(N, F, T) as plan:
+        assert plan.info["path"] == corr.PATH_IMMA
+        assert plan.info["slices"] >= 2, plan.info
+        dev = torch.zeros((T, F, N), dtype=torch.uint8, device="cuda")
+        vis = plan.new_vis()
+        vis.fill_(-559038737)
+        plan.execute(dev, vis)
+        torch.cuda.synchronize()
+        assert bool((vis[..., 0] == 128 * T).all()) and bool((vis[..., 1] == 0).all())
+        dev.fill_(0xFF)                                   # +7+7i: Re = 98 T
+        plan.execute(dev, vis, accumulate=True)
+        torch.cuda.synchronize()
+        assert bool((vis[..., 0] == (128 + 98) * T).all()) and bool((vis[..., 1] == 0).all())
+
+
+def test_concurrent_plans_with_cut_units(corr, oracle):
+    # Two plans whose units are all cut into pieces (4 and 6 units on 74 CTA pairs), run at the same time on two
+    # streams, and again while an unrelated long kernel holds part of the GPU: the pieces of a cut unit order
+    # their store through a claim flag that only ever waits for a CTA that is already running, so this must
+    # finish (it would hang if a piece waited for a CTA that is not resident) and be bit-exact.
+    import torch
+    shapes = [(256, 2, 20000, 301), (384, 1, 12000, 302)]
+    packs = [workloads.iid_gaussian(N, F, T, seed=sd) for (N, F, T, sd) in shapes]
+    wants = [oracle.level1(pk) for pk in packs]
+    plans = [corr.Plan(N, F, T, corr.PATH_TCGEN05) for (N, F, T, _) in shapes]
+    try:
+        devs = [torch.from_numpy(pk).cuda() for pk in packs]
+        viss = [pl.new_vis() for pl in plans]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        busy = torch.cuda.Stream()
+        a = torch.randn(4096, 4096, device="cuda")
+        torch.cuda.synchronize()
+        for rep in range(6):
+            for v in viss:
+                v.fill_(-559038737)
+            torch.cuda.synchronize()
+            if rep >= 3:
+                with torch.cuda.stream(busy):
+                    for _ in range(4):
+                        a = torch.tanh(a) * 1.0001        # elementwise kernels with many small CTAs
+            for k in range(4):
+                for pl, d, v, st in zip(plans, devs, viss, streams):
+                    pl.execute(d, v, stream=st)
+            torch.cuda.synchronize()
+            for v, w, sh in zip(viss, wants, shapes):
+                assert np.array_equal(v.cpu().numpy(), w), (sh, rep)
+    finally:
+        for pl in plans:
+            pl.close()
+
+
 @pytest.mark.parametrize("case", [(272, 3, 700, "TCGEN05"), (2048, 1, 300, "TCGEN05"), (400, 2, 520, "TCGEN05"),
                                   (16, 9, 3000, "IMMA"), (64, 3, 1300, "IMMA"), (100, 2, 300, "DP4A"), (17, 3, 65, "DP4A")])
 def test_no_write_outside_the_output(corr, oracle, case):
