@@ -35,7 +35,7 @@ NOMINAL_INT8_TOPS = 4500.0  # dense int8 = 2x dense bf16 2250 (B200_PROFILING.md
 # roofline.traffic comes from a tracked ncu summary (profiles/), which records the kernel it was captured on and
 # the SHA-256 of that kernel's sources at capture time; a stale record (sources changed since) reports null.
 TRAFFIC_RECORD = ROOT / "profiles" / "tc_traffic.txt"
-KERNEL_SOURCES = ("corr_tc3.cuh", "corr_tc4.cuh", "corr_ptx.cuh", "corr_api.cu")
+KERNEL_SOURCES = ("corr_tc3.cuh", "corr_tc5.cuh", "corr_tc.cuh", "corr_ptx.cuh", "corr_api.cu")
 
 # the N sweep of the paper's Fig. 4 axis (inputs >= 256 MB for small N so that GB/s means something)
 # and the five BASELINE.json shapes: (label, N, F, T, accumulate)
@@ -356,7 +356,7 @@ def main():
     int8_measured = corr.corr_measure_int8_tops(20000)
     if path == corr.PATH_TCGEN05:
         variant = os.environ.get("CORR_TC_VARIANT", "3")
-        kernel = {"1": "corr_tc_kernel", "2": "corr_tc2_kernel", "4": "corr_tc4_kernel"}.get(variant, "corr_tc3_kernel")
+        kernel = {"1": "corr_tc_kernel", "5": "corr_tc5_kernel"}.get(variant, "corr_tc3_kernel")
         traffic, traffic_source = recorded_traffic(kernel, args.config)
         roofline = {
             "bound": "tensor", "achieved": achieved, "peak": int8_peak, "unit": "TOP/s", "frac": achieved / int8_peak,

@@ -5,6 +5,7 @@ to the GPU box.
 """
 from __future__ import annotations
 
+import os
 import subprocess
 import sys
 from pathlib import Path
@@ -26,7 +27,9 @@ NVCC_FLAGS = [
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and LIB.exists() and all(LIB.stat().st_mtime >= d.stat().st_mtime for d in DEPS):
         return LIB
-    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *map(str, SOURCES), "-o", str(LIB)]
+    extra = os.environ.get("CORR_NVCC_EXTRA", "").split()   # e.g. -DT5_PK_N=4 (kernel tuning experiments)
+    out = Path(os.environ.get("CORR_LIB_OUT", str(LIB)))
+    cmd = ["nvcc", *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), *map(str, SOURCES), "-o", str(out)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

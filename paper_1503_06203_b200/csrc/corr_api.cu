@@ -19,9 +19,8 @@
 #include "corr_peak.cuh"
 #include "corr_shift.cuh"
 #include "corr_tc.cuh"
-#include "corr_tc2.cuh"
 #include "corr_tc3.cuh"
-#include "corr_tc4.cuh"
+#include "corr_tc5.cuh"
 
 namespace {
 
@@ -78,6 +77,54 @@ int count_tiles(int N, int tx, int ty)
 
 }  // namespace
 
+// S3, the tail of the schedule (corr_tc3.cuh): the units left after the last whole wave are cut into pieces, one or
+// two per CTA pair, so that every pair finishes at the same time.  The cost of a pair is counted in groups of
+// T3_GROUP samples: its pieces, a fixed cost per piece (accumulator drain, epilogue, and the output being summed in
+// memory) and the extra time its transposed tiles take in the epilogue (measured: ~3 and ~3.5 groups).  The first
+// piece of a cut unit is marked EARLY: its pair computes it before its whole units, so that its store is long done
+// when the other pieces add theirs.  Pieces are handed out in unit order, pair by pair, for the smallest budget
+// (binary search) that places every group.
+static void tc3_build_pieces(int num_units, int npairs, int slices, int groups_full, int groups_last,
+                             const std::vector<ushort4> &tiles4, std::vector<int4> &pieces)
+{
+    const double E = 3.0, XT = 3.5;
+    const int tiles_per_f = (int)tiles4.size();
+    pieces.assign((size_t)npairs * corr::TC3_MAX_PIECES, make_int4(0, 0, 0, 0));
+    const int waves = num_units / npairs, u0 = waves * npairs;
+    if (u0 == num_units) return;
+    auto len = [&](int u) { return (u % slices == slices - 1) ? groups_last : groups_full; };
+    auto transposed = [&](int u) { return (tiles4[(size_t)((u / slices) % tiles_per_f)].w & corr::TC3_TILE_TRANSPOSED) != 0; };
+    std::vector<double> pre((size_t)npairs, 0.0);
+    double gt = 0.0;
+    for (int pr = 0; pr < npairs; ++pr)
+        for (int k = 0; k < waves; ++k)
+            if (transposed(pr + k * npairs)) pre[(size_t)pr] += XT;
+    for (int u = u0; u < num_units; ++u) gt += len(u);
+    auto assign = [&](double B, bool commit) {
+        int u = u0, off = 0;
+        for (int pr = 0; pr < npairs && u < num_units; ++pr) {
+            double budget = B - pre[(size_t)pr];
+            for (int np = 0; np < corr::TC3_MAX_PIECES && u < num_units; ++np) {
+                const int room = (int)(budget - E);
+                if (room < 1) break;
+                const int l = len(u), cnt = std::min(l - off, room);
+                if (commit)
+                    pieces[(size_t)pr * corr::TC3_MAX_PIECES + np] = make_int4(u, off, cnt, (off == 0 && cnt < l && waves > 0) ? 1 : 0);
+                budget -= cnt + E + (transposed(u) ? XT * cnt / l : 0.0);
+                off += cnt;
+                if (off == l) { ++u; off = 0; }
+            }
+        }
+        return u == num_units;
+    };
+    double lo = 0.0, hi = gt + 2.0 * (E + XT) * corr::TC3_MAX_PIECES + 64.0;
+    for (int it = 0; it < 48; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (assign(mid, false)) hi = mid; else lo = mid;
+    }
+    assign(hi, true);
+}
+
 static bool alloc_pad_buf(struct corr_plan *p);
 
 struct corr_plan {
@@ -98,13 +145,13 @@ struct corr_plan {
     // dp4a only
     int aligned;
     // tcgen05 only
-    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh); 2: CTA-pair tiles 256x128, operands in smem
-                       // (corr_tc2.cuh); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
-                       // 4: as 3 with three products per complex MAC (corr_tc4.cuh; CORR_TC_VARIANT=4)
+    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh; chosen for N <= 128, where a pair tile would be
+                       // half empty); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
+                       // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
     int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
     long long total_groups;
     int *flags_dev;    // variant 3: [num_units][2] stream-K flags (corr_tc3.cuh)
-    int32_t *sums_dev; // variant 4: [2][slices][F][N] per-element sums of the stored bytes
+    int4 *pieces_dev;  // variant 3: [pairs][TC3_MAX_PIECES] tail pieces of every CTA pair (tc3_build_pieces)
     CUtensorMap tmap;
     CUtensorMap tmap_y;
     const void *tmap_ptr;
@@ -166,7 +213,7 @@ int corr_plan_info(const corr_plan *p, int info[8])
         return CORR_ERR_INVALID_ARG;
     }
     info[0] = p->path;
-    info[1] = (p->variant >= 2) ? 256 : p->tile;
+    info[1] = (p->variant >= 3) ? 256 : p->tile;
     info[2] = p->tile;
     info[3] = p->tiles_per_f;
     info[4] = p->slices;
@@ -182,8 +229,8 @@ void corr_plan_destroy(corr_plan *p)
     if (p->pad_buf) cudaFree(p->pad_buf);
     if (p->tiles_dev) cudaFree(p->tiles_dev);
     if (p->tiles4_dev) cudaFree(p->tiles4_dev);
-    if (p->sums_dev) cudaFree(p->sums_dev);
     if (p->flags_dev) cudaFree(p->flags_dev);
+    if (p->pieces_dev) cudaFree(p->pieces_dev);
     if (p->host_fg != 0) cudaEventDestroy(p->ev_done);
     if (p->gate_plans) {
         for (auto &kv : *p->gate_plans) corr_plan_destroy(kv.second);
@@ -325,19 +372,15 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->tile = corr::TC_BLK;
     p->variant = 0;
     if (path == CORR_PATH_TCGEN05) {
-        const char *v = getenv("CORR_TC_VARIANT");
-        p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "2")) ? 2 : (v && !strcmp(v, "4")) ? 4 : 3;
-        if (p->variant != 3 && n_pad != N) {
-            g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: CORR_TC_VARIANT=%d needs N %% 16 == 0 (only the default kernel reads a padded stream), got N=%d",
-                    p->variant, N);
-            delete p;
-            return nullptr;
-        }
+        // N <= 128 is one 128-block per channel: a CTA-pair tile would have an idle half (measured 923 against 1358
+        // effective TOPS at N = 128, profiles/r02_sweep.md), so single-CTA tiles take over there
+        const char *v = getenv("CORR_TC_VARIANT");   // testing aid: force a kernel
+        p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "3")) ? 3 : (v && !strcmp(v, "5")) ? 5 : (n_pad <= 128) ? 1 : 3;
     }
     const int nb = (N + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
     std::vector<ushort4> tiles4;
-    if (p->variant == 3) {
+    if (p->variant >= 3) {
         // Pair tiles of two row blocks (128 inputs each) against one column block.  Column block j needs the row
         // blocks 0..j.  An even count pairs up as (0,1), (2,3), ...; an odd count as (1,2), (3,4), ... and leaves
         // block (0, j) over.  The left-over blocks all have row block 0: computed transposed (rows = block j,
@@ -353,12 +396,6 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             tiles4.push_back(make_ushort4(us(left[i]), (i + 1 < left.size()) ? us(left[i + 1]) : corr::TC3_NO_BLOCK, 0,
                                           corr::TC3_TILE_TRANSPOSED));
         tiles.resize(tiles4.size());   // the count is what the schedule below needs
-    } else if (p->variant >= 2) {
-        // pair tiles: x-block of 256 (two CTAs x 128), y-block of 128; keep those whose largest y
-        // reaches their smallest x
-        const int nbx = (N + 255) / 256;
-        for (int bx = 0; bx < nbx; ++bx)
-            for (int by = 2 * bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
     } else {
         for (int bx = 0; bx < nb; ++bx)
             for (int by = bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
@@ -373,18 +410,17 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
 
     // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
     const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK
-                        : (p->variant == 4) ? corr::T4_GROUP
-                        : (p->variant == 3) ? corr::T3_ST * corr::T3_PL_STAGES  // tc3 / tc4 run whole groups of stages
+                        : (p->variant >= 3) ? corr::T3_GROUP  // tc3 / tc5 run whole groups of stages
                                             : corr::TC_ST;
-    const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : (p->variant == 4) ? corr::T4_MAX_SLICE : corr::TC_MAX_SLICE;
-    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant >= 2 ? p->sm_count / 2 : p->sm_count);
+    const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : (p->variant == 5) ? corr::T5_MAX_SLICE : corr::TC_MAX_SLICE;
+    const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant >= 3 ? p->sm_count / 2 : p->sm_count);
     const double per_sample = (path == CORR_PATH_DP4A) ? 40.0 : 8.0;  // cycles per time sample per unit
     const double epi = (path == CORR_PATH_DP4A) ? 1500.0 : 6000.0;    // cycles per unit, fixed
     const int min_slices = (T + max_slice - 1) / max_slice;
     double best_cost = 0;
     int best_s = 0;
     // variant 3 balances the load itself (stream-K over groups of stages): T is split only for int32 headroom
-    const int s_max = (p->variant == 3) ? min_slices : std::max(min_slices, 64);
+    const int s_max = (p->variant >= 3) ? min_slices : std::max(min_slices, 64);
     for (int s = min_slices; s <= s_max; ++s) {
         int tps = ((T + s - 1) / s + quantum - 1) / quantum * quantum;
         if (s > min_slices && tps < 8 * quantum) break;
@@ -400,17 +436,21 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->slices = (T + p->t_per_slice - 1) / p->t_per_slice;
     p->num_units = (int)(units0 * p->slices);
     p->grid = (path == CORR_PATH_DP4A) ? p->num_units
-              : (p->variant >= 2) ? 2 * std::min(p->num_units, p->sm_count / 2)
+              : (p->variant >= 3) ? 2 * std::min(p->num_units, p->sm_count / 2)
                                   : std::min(p->num_units, p->sm_count);
-    p->kernels_per_exec = ((p->variant == 4) ? 2 : 1) + ((path != CORR_PATH_DP4A && n_pad != N) ? 1 : 0);  // tc4: + corr_sums_kernel; + corr_pad_kernel
+    p->kernels_per_exec = 1 + ((path != CORR_PATH_DP4A && n_pad != N) ? 1 : 0);  // + corr_pad_kernel
     p->aligned = (N % 4 == 0) ? 1 : 0;
-    if (p->variant == 3) {
+    if (p->variant >= 3) {
         p->groups_full = p->t_per_slice / corr::T3_GROUP;
         p->groups_last = (T - (p->slices - 1) * p->t_per_slice + corr::T3_GROUP - 1) / corr::T3_GROUP;
         p->total_groups = units0 * ((long long)(p->slices - 1) * p->groups_full + p->groups_last);
         p->grid = 2 * (int)std::min<long long>(p->total_groups, p->sm_count / 2);
+        std::vector<int4> pieces;
+        tc3_build_pieces(p->num_units, p->grid / 2, p->slices, p->groups_full, p->groups_last, tiles4, pieces);
         if (cudaMalloc(&p->flags_dev, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess ||
-            cudaMemset(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess) {
+            cudaMemset(p->flags_dev, 0, (2 * (size_t)p->num_units + 1) * sizeof(int)) != cudaSuccess ||
+            cudaMalloc(&p->pieces_dev, pieces.size() * sizeof(int4)) != cudaSuccess ||
+            cudaMemcpy(p->pieces_dev, pieces.data(), pieces.size() * sizeof(int4), cudaMemcpyHostToDevice) != cudaSuccess) {
             g_create_rc = CORR_ERR_ALLOC; set_err("corr_plan_create: device allocation of the schedule flags failed: %s",
                     cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
@@ -436,18 +476,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         }
         cudaError_t e1 = cudaFuncSetAttribute(corr::corr_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::TC_SMEM_BYTES);
-        cudaError_t e2 = cudaFuncSetAttribute(corr::corr_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                              corr::T2_SMEM_BYTES);
         cudaError_t e3 = cudaFuncSetAttribute(corr::corr_tc3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::T3_SMEM_BYTES);
-        if (e3 == cudaSuccess)
-            e3 = cudaFuncSetAttribute(corr::corr_tc4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      corr::T4_SMEM_BYTES);
-        if (e3 == cudaSuccess && p->variant == 4)
-            e3 = cudaMalloc(&p->sums_dev, 2 * (size_t)p->slices * F * N * sizeof(int32_t));
-        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+        cudaError_t e5 = cudaFuncSetAttribute(corr::corr_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              corr::T5_SMEM_BYTES);
+        if (e1 != cudaSuccess || e3 != cudaSuccess || e5 != cudaSuccess) {
             g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
-                    corr::T2_SMEM_BYTES, corr::T3_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
+                    corr::T3_SMEM_BYTES, corr::T5_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
             corr_plan_destroy(p);
             return nullptr;
         }
@@ -540,12 +575,12 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     const cuuint64_t dims[3] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F, (cuuint64_t)p->T};
     const cuuint64_t strides[2] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F * (cuuint64_t)p->n_pad};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const int st = (p->variant == 4) ? corr::T4_ST : (p->variant == 3) ? corr::T3_ST : (p->variant == 2) ? corr::T2_ST : corr::TC_ST;
+    const int st = (p->variant >= 3) ? corr::T3_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r == CUDA_SUCCESS && p->variant >= 2) {
+    if (r == CUDA_SUCCESS && p->variant >= 3) {
         const cuuint32_t boxy[3] = {64u, 1u, (cuuint32_t)st};  // half a y-block per CTA of the pair
         r = get_encode_fn()(&p->tmap_y, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                             strides, boxy, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
@@ -626,30 +661,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     } else {
         int rc = build_tmap(p, packed_dev);
         if (rc != CORR_OK) return rc;
-        if (p->variant == 4) {
-            // per-element sums of the stored bytes over every slice, then the 3-product kernel
-            const size_t nsum = (size_t)p->slices * p->F * p->N;
-            CUDA_TRY(cudaMemsetAsync(p->sums_dev, 0, 2 * nsum * sizeof(int32_t), stream), CORR_ERR_CUDA);
-            const int rows_per_block = corr::sums_rows_per_block(p->N);
-            dim3 sgrid((unsigned)((p->t_per_slice + rows_per_block - 1) / rows_per_block), (unsigned)p->F,
-                       (unsigned)p->slices);
-            corr::corr_sums_kernel<<<sgrid, corr::SUMS_THREADS, 0, stream>>>(packed_dev, p->sums_dev, p->sums_dev + nsum,
-                                                                             p->N, p->F, p->T, p->t_per_slice);
-            corr::Tc4Params prm;
-            prm.N = p->N;
-            prm.F = p->F;
-            prm.T = p->T;
-            prm.tiles_per_f = p->tiles_per_f;
-            prm.slices = p->slices;
-            prm.t_per_slice = p->t_per_slice;
-            prm.num_units = p->num_units;
-            prm.out_mode = out_mode;
-            prm.tiles = p->tiles_dev;
-            prm.sum_w = p->sums_dev;
-            prm.sum_lo = p->sums_dev + nsum;
-            prm.vis = vis_dev;
-            corr::corr_tc4_kernel<<<p->grid, corr::T4_THREADS, corr::T4_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
-        } else if (p->variant == 3) {
+        if (p->variant >= 3) {
             corr::Tc3Params prm;
             prm.N = p->N;
             prm.F = p->F;
@@ -663,22 +675,13 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.groups_last = p->groups_last;
             prm.total_groups = p->total_groups;
             prm.flags = p->flags_dev;
+            prm.pieces = p->pieces_dev;
             prm.tiles = p->tiles4_dev;
             prm.vis = vis_dev;
-            corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
-        } else if (p->variant == 2) {
-            corr::Tc2Params prm;
-            prm.N = p->N;
-            prm.F = p->F;
-            prm.T = p->T;
-            prm.tiles_per_f = p->tiles_per_f;
-            prm.slices = p->slices;
-            prm.t_per_slice = p->t_per_slice;
-            prm.num_units = p->num_units;
-            prm.out_mode = out_mode;
-            prm.tiles = p->tiles_dev;
-            prm.vis = vis_dev;
-            corr::corr_tc2_kernel<<<p->grid, corr::T2_THREADS, corr::T2_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+            if (p->variant == 5)
+                corr::corr_tc5_kernel<<<p->grid, corr::T5_THREADS, corr::T5_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+            else
+                corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
         } else {
             corr::TcParams prm;
             prm.N = p->N;

@@ -75,6 +75,7 @@ struct Tc3Params {
     long long total_groups;  // over all units
     int *flags;        // [num_units][2]: claim / stored state of (unit, CTA rank), see tc3_claim_store;
                        // [2 * num_units]: CTAs that have finished (the last one clears the array for the next launch)
+    const int4 *pieces;    // [pairs][TC3_MAX_PIECES]: the tail pieces of every pair, see Tc3Iter
     const ushort4 *tiles;  // (xa, xb, by, flags): 128-blocks of the rows of CTA 0 and CTA 1, of the columns; see Tc3Tile
     int32_t *vis;
 };
@@ -100,9 +101,15 @@ struct Tc3Seg {
     int t_begin, t_end;    // first sample of the segment; end of the unit's slice (<= T)
 };
 
+// The pieces of the tail units that a pair computes (host: tc3_build_pieces in corr_api.cu): (unit, first group,
+// number of groups, early).  An EARLY piece is the first piece of a cut unit and is computed BEFORE the pair's whole
+// units: it stores its partial sums hundreds of microseconds before the other pieces of that unit (computed after
+// the whole units) add theirs, so nobody waits for anybody at the end of the kernel.
+constexpr int TC3_MAX_PIECES = 4;
+
 struct Tc3Iter {
     int k, waves, pair, npairs;
-    long long g, g_end;
+    int phase, pi;         // 0: early pieces, 1: whole units, 2: late pieces; next piece entry
 };
 
 __device__ __forceinline__ Tc3Iter tc3_iter(const Tc3Params &p, int pair, int npairs)
@@ -112,42 +119,49 @@ __device__ __forceinline__ Tc3Iter tc3_iter(const Tc3Params &p, int pair, int np
     it.waves = p.num_units / npairs;
     it.pair = pair;
     it.npairs = npairs;
-    // first group of the first tail unit in the linear order of units
-    const int u0 = it.waves * npairs;
-    const int full = (p.slices - 1) * p.groups_full;
-    const long long g0 = (long long)(u0 / p.slices) * (full + p.groups_last) + (long long)(u0 % p.slices) * p.groups_full;
-    const long long tail = p.total_groups - g0;
-    it.g = g0 + tail * pair / npairs;
-    it.g_end = g0 + tail * (pair + 1) / npairs;
+    it.phase = 0;
+    it.pi = 0;
     return it;
 }
 
 __device__ __forceinline__ bool tc3_next_segment(const Tc3Params &p, Tc3Iter &it, Tc3Seg &s)
 {
-    const int full = (p.slices - 1) * p.groups_full;
-    const int per_ft = full + p.groups_last;
-    long long ft;
-    if (it.k < it.waves) {               // a whole unit of a whole wave
-        const int u = it.pair + it.k * it.npairs;
-        ++it.k;
-        ft = u / p.slices;
-        s.slice = u % p.slices;
-        s.first = 0;
-        s.len = (s.slice == p.slices - 1) ? p.groups_last : p.groups_full;
-        s.cnt = s.len;
-    } else {                             // this pair's share of the tail units
-        if (it.g >= it.g_end) return false;
-        ft = it.g / per_ft;
-        const int r = (int)(it.g - ft * per_ft);
-        s.slice = (r < full) ? r / p.groups_full : p.slices - 1;
-        s.first = r - s.slice * p.groups_full;
-        s.len = (s.slice == p.slices - 1) ? p.groups_last : p.groups_full;
-        s.cnt = (int)min((long long)(s.len - s.first), it.g_end - it.g);
-        it.g += s.cnt;
+    int u;
+    for (;;) {
+        if (it.phase == 1) {                 // a whole unit of a whole wave
+            if (it.k < it.waves) {
+                u = it.pair + it.k * it.npairs;
+                ++it.k;
+                s.first = 0;
+                s.cnt = -1;
+                break;
+            }
+            it.phase = 2;
+            it.pi = 0;
+        } else {                             // this pair's pieces of the tail units
+            bool found = false;
+            while (it.pi < TC3_MAX_PIECES) {
+                const int4 e = p.pieces[it.pair * TC3_MAX_PIECES + it.pi++];
+                if (e.z > 0 && (e.w != 0) == (it.phase == 0)) {
+                    u = e.x;
+                    s.first = e.y;
+                    s.cnt = e.z;
+                    found = true;
+                    break;
+                }
+            }
+            if (found) break;
+            if (it.phase == 2) return false;
+            it.phase = 1;
+        }
     }
-    s.f = (int)(ft / p.tiles_per_f);
-    s.tile = p.tiles[(int)(ft % p.tiles_per_f)];
-    s.u = (int)ft * p.slices + s.slice;
+    const int ft = u / p.slices;
+    s.slice = u - ft * p.slices;
+    s.len = (s.slice == p.slices - 1) ? p.groups_last : p.groups_full;
+    if (s.cnt < 0) s.cnt = s.len;
+    s.f = ft / p.tiles_per_f;
+    s.tile = p.tiles[ft - s.f * p.tiles_per_f];
+    s.u = u;
     s.t_begin = s.slice * p.t_per_slice + s.first * T3_GROUP;
     s.t_end = min(p.T, (s.slice + 1) * p.t_per_slice);
     return true;
@@ -158,12 +172,13 @@ constexpr int TC3_FLAG_CLAIMED = 1, TC3_FLAG_STORED = 2;
 
 // Called by all epilogue threads of a CTA (warp-uniform control flow).  Returns true in the CTA whose piece
 // stores (the first to arrive); in every other CTA it returns, false, once the store is visible.
-__device__ __forceinline__ bool tc3_claim_store(int *flag, volatile int *claim_smem)
+__device__ __forceinline__ bool tc3_claim_store(int *flag, volatile int *claim_smem, int epi_thread0 = 32 * T3_EPI_WARP0,
+                                                int epi_threads = 32 * T3_EPI_WARPS)
 {
-    if (threadIdx.x == 32 * T3_EPI_WARP0) *claim_smem = atomicCAS(flag, 0, TC3_FLAG_CLAIMED);
-    ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);
+    if ((int)threadIdx.x == epi_thread0) *claim_smem = atomicCAS(flag, 0, TC3_FLAG_CLAIMED);
+    ptx::named_bar_sync(1, epi_threads);
     const int before = *claim_smem;
-    ptx::named_bar_sync(1, 32 * T3_EPI_WARPS);   // everyone has read the slot before its next use
+    ptx::named_bar_sync(1, epi_threads);   // everyone has read the slot before its next use
     if (before == 0) return true;
     while (ptx::ld_acquire_gpu(flag) != TC3_FLAG_STORED) {
     }

@@ -180,13 +180,15 @@ def test_determinism(corr):
     assert np.array_equal(_run(corr, packed, corr.PATH_IMMA)[0], _run(corr, packed, corr.PATH_TCGEN05)[0])
 
 
-@pytest.mark.parametrize("variant", ["1", "2", "3", "4"])
+@pytest.mark.parametrize("variant", ["1", "3", "5"])
 def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
-    # CORR_TC_VARIANT selects the kernel at plan creation: 1 single-CTA tiles, 2 CTA pair with both
-    # operands in shared memory, 3 A operand in TMEM (default), 4 three products per complex MAC
-    # (offset route, Eq. 3).  Same bits from all of them, including ragged N, split T and accumulation.
+    # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles (automatic for N <= 128), 3 CTA pair
+    # with the A operand in TMEM (automatic above), 5 three products per complex MAC on the stored bytes with
+    # fused per-element sums (offset route, Eq. 3).  Same bits from all of them, including ragged N (also
+    # N % 16 != 0 through the padded stream), split T, cut units and accumulation.
     monkeypatch.setenv("CORR_TC_VARIANT", variant)
-    for (N, F, T, seed) in [(272, 3, 1000, 11), (1024, 2, 333, 12), (256, 1, 40000, 13), (2048, 1, 640, 14)]:
+    for (N, F, T, seed) in [(272, 3, 1000, 11), (1024, 2, 333, 12), (256, 1, 40000, 13), (2048, 1, 640, 14), (100, 3, 500, 15),
+                            (400, 2, 777, 16), (512, 4, 8192, 17)]:
         packed = workloads.uniform_bytes(N, F, T, seed=seed)
         want = oracle.level1(packed)
         got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=-559038737)
@@ -406,7 +408,7 @@ def test_no_write_outside_the_output(corr, oracle, case):
     packed = workloads.uniform_bytes(N, F, T, seed=N * 3 + T)
     want = oracle.level1(packed)
     G = 256   # guard ints (1 KB keeps vis 16-byte aligned)
-    for variant in (("3", "4") if path == "TCGEN05" else ("3",)):
+    for variant in (("1", "3", "5") if path == "TCGEN05" else ("3",)):
         import os
         os.environ["CORR_TC_VARIANT"] = variant
         try:
@@ -444,10 +446,10 @@ def test_invalid_arguments(corr):
 
 
 # ------------------------------------------------------------------ the five BASELINE.json configs
-def _config_case(corr, oracle, name):
+def _config_case(corr, oracle, name, path=0):
     import torch
     cfg = workloads.CONFIGS[name]
-    with corr.Plan(cfg.N, cfg.F, cfg.T) as plan:
+    with corr.Plan(cfg.N, cfg.F, cfg.T, path) as plan:
         vis = plan.new_vis()
         vis.fill_(-1)
         want = None
@@ -479,6 +481,14 @@ def test_cfg4(corr, oracle):
 
 def test_cfg5(corr, oracle):
     _config_case(corr, oracle, "cfg5")
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg5"])
+def test_configs_on_the_three_product_kernel(corr, oracle, name, monkeypatch):
+    # the BASELINE.json shapes through corr_tc5_kernel (three products per complex MAC, fused per-element sums):
+    # cfg1 is 16 inputs padded into one 128-block, cfg2 runs only cut units, cfg5 accumulates over eight calls
+    monkeypatch.setenv("CORR_TC_VARIANT", "5")
+    _config_case(corr, oracle, name, corr.PATH_TCGEN05)
 
 
 def test_cfg5_memset_then_eight_accumulates(corr, oracle):
