@@ -80,14 +80,15 @@ int count_tiles(int N, int tx, int ty)
 // S3, the tail of the schedule (corr_tc3.cuh): the units left after the last whole wave are cut into pieces, one or
 // two per CTA pair, so that every pair finishes at the same time.  The cost of a pair is counted in groups of
 // T3_GROUP samples: its pieces, a fixed cost per piece (accumulator drain, epilogue, and the output being summed in
-// memory) and the extra time its transposed tiles take in the epilogue (measured: ~3 and ~3.5 groups).  The first
+// memory) and the extra time its transposed tiles take in the epilogue (~3 and ~0.5 groups; the result is flat
+// within 0.3 % for 2..5 and 0..3.5, profiles/r02_tc3_ncu_summary.md).  The first
 // piece of a cut unit is marked EARLY: its pair computes it before its whole units, so that its store is long done
 // when the other pieces add theirs.  Pieces are handed out in unit order, pair by pair, for the smallest budget
 // (binary search) that places every group.
 static void tc3_build_pieces(int num_units, int npairs, int slices, int groups_full, int groups_last,
                              const std::vector<ushort4> &tiles4, std::vector<int4> &pieces)
 {
-    const double E = 3.0, XT = 3.5;
+    const double E = 3.0, XT = 0.5;
     const int tiles_per_f = (int)tiles4.size();
     pieces.assign((size_t)npairs * corr::TC3_MAX_PIECES, make_int4(0, 0, 0, 0));
     const int waves = num_units / npairs, u0 = waves * npairs;

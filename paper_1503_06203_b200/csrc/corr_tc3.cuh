@@ -395,6 +395,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         const long long Bn = (long long)p.N * ((long long)p.N + 1) / 2;
         const bool base_add = (p.out_mode != OUT_STORE);
         uint32_t acc_ph = 0;
+        bool prev_transposed = false;
         while (tc3_next_segment(p, sit, sg)) {
             // A unit cut by the stream-K schedule is summed in memory.  When the call overwrites (OUT_STORE),
             // the piece that gets to its output FIRST claims the unit (atomic compare-and-swap on the unit's flag),
@@ -410,15 +411,22 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             const int xw = x0 + q * 32;
             const int x = x0 + row;
             const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
-            if (tile.w & TC3_TILE_TRANSPOSED) {
-                // ---- transposed block: this thread's MMA row is the baseline's y, the MMA columns are its x.
-                // vis(x', y') = conj(D[y'][x']); for one column the 32 lanes of a warp hold consecutive y', which
-                // are consecutive in vis: every store instruction writes one contiguous 256-byte run.
+            const bool transposed = (tile.w & TC3_TILE_TRANSPOSED) != 0;
+            if (transposed || prev_transposed) {
+                // a transposed unit's row images are written by all epilogue threads and sent by others: everybody's
+                // previous copies must have left shared memory before anybody writes
+                ptx::bulk_wait_read0();
+                ptx::named_bar_sync(3, 32 * T3_EPI_WARPS);
+            }
+            prev_transposed = transposed;
+            if (transposed) {
+                // ---- transposed block: this thread's MMA row is the baseline's y, the MMA columns are its x,
+                // vis(x', y') = conj(D[y'][x']).  For one MMA column the 32 lanes of a warp hold consecutive y', which
+                // are consecutive in vis: the image of output row x' = y0 + c is shared-memory row c, written by
+                // the lanes side by side (conflict-free), and thread c of the h = 0 warps sends it as one bulk copy.
                 ptx::mbar_wait_cluster(acc_full, acc_ph);
                 acc_ph ^= 1u;
                 ptx::tc_fence_after_sync();
-                if (claim) add = !tc3_claim_store(flag, claim_g), raise_flag = !add;
-                const int yt = x;   // true y of this thread
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const int col = 64 * h + 16 * c;
@@ -433,20 +441,48 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
 #pragma unroll
                         for (int j = 0; j < 16; ++j) {
                             const int xt = xt0 + j;
-                            if (yt < p.N && xt <= yt) {
-                                const int re = (int)rr[j] >> 8;
-                                const int im = -((int)(ir[j] - ri[j]) >> 8);
-                                int2 *o = reinterpret_cast<int2 *>(p.vis) + (long long)f * Bn + (long long)xt * p.N -
-                                          (long long)xt * (xt - 1) / 2 + (yt - xt);
-                                if (add) { atomicAdd(&o->x, re); atomicAdd(&o->y, im); }
-                                else *o = make_int2(re, im);
-                            }
+                            // parity of the 8-byte index of (xt, x0) in vis: slot of MMA row R in image row col + j
+                            const long long gi = (long long)f * Bn + (long long)xt * p.N - (long long)xt * (xt - 1) / 2 - xt + x0;
+                            const uint32_t parc = (uint32_t)((reinterpret_cast<uintptr_t>(p.vis) >> 3) + (unsigned long long)gi) & 1u;
+                            const int re = (int)rr[j] >> 8;
+                            const int im = -((int)(ir[j] - ri[j]) >> 8);
+                            *reinterpret_cast<int2 *>(epi_g + (col + j) * T3_EPI_PITCH + 8 * (parc + row)) = make_int2(re, im);
                         }
                     }
                 }
+                // TMEM is free for the next unit
                 ptx::tc_fence_before_sync();
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive_cluster(acc_empty, 0);
+                if (claim) add = !tc3_claim_store(flag, claim_g), raise_flag = !add;
+                ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
+                ptx::named_bar_sync(3, 32 * T3_EPI_WARPS);   // every image row is complete
+                if (h == 0) {
+                    // image row `row` = output row xt, columns yt = x0 + R for R in [rlo, rhi)
+                    const int xt = y0 + row;
+                    int rlo = max(0, xt - x0), rhi = min(128, p.N - x0);
+                    if (xt < p.N && rlo < rhi) {
+                        const long long gi = (long long)f * Bn + (long long)xt * p.N - (long long)xt * (xt - 1) / 2 - xt + x0;
+                        int2 *grow = reinterpret_cast<int2 *>(p.vis) + gi;
+                        const uint32_t parc = (uint32_t)(reinterpret_cast<uintptr_t>(grow) >> 3) & 1u;
+                        if ((parc + rlo) & 1) {           // leading baseline on an odd 8-byte slot
+                            const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * (parc + rlo));
+                            if (add) { atomicAdd(&grow[rlo].x, v.x); atomicAdd(&grow[rlo].y, v.y); }
+                            else grow[rlo] = v;
+                            ++rlo;
+                        }
+                        if ((rhi - rlo) & 1) {            // trailing baseline
+                            --rhi;
+                            const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * (parc + rhi));
+                            if (add) { atomicAdd(&grow[rhi].x, v.x); atomicAdd(&grow[rhi].y, v.y); }
+                            else grow[rhi] = v;
+                        }
+                        if (rlo < rhi) {
+                            if (add) ptx::bulk_reduce_add_s32(grow + rlo, srow + 8u * (parc + rlo), 8u * (rhi - rlo));
+                            else ptx::bulk_store(grow + rlo, srow + 8u * (parc + rlo), 8u * (rhi - rlo));
+                        }
+                    }
+                }
             } else {
             // 8-byte index of (x, y0) in vis (formal when y0 < x: only its parity and offsets from it are used)
             const long long g0 = (long long)f * Bn + (long long)x * p.N - (long long)x * (x - 1) / 2 - x + y0;
