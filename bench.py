@@ -340,6 +340,30 @@ def main():
     e2e_blocking_s = (time.perf_counter() - t0) / args.e2e_steps
     e2e_s = shard.max_over_ranks(e2e_s, dev)
     e2e_value = eff_ops(N, F, T) * world / e2e_s / 1e12
+    # ---- what the host link gives on this box (PAPER.md:129 lower panel is the paper's own I/O concern): one pinned
+    #      copy of the step's input in, one of its output out, alone and both at once on two streams
+    link = None
+    if world == 1:
+        s_a, s_b = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        d_in, d_out = torch.empty_like(dev_inputs[0]), vis
+        def timed(h2d, d2h):
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            if h2d:
+                with torch.cuda.stream(s_a):
+                    d_in.copy_(ph[0], non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s_b):
+                    vhs[1].copy_(d_out, non_blocking=True)
+            torch.cuda.synchronize(dev)
+            return time.perf_counter() - t0
+        for _ in range(2):
+            t_in, t_out, t_both = timed(True, False), timed(False, True), timed(True, True)
+        b_in, b_out = float(N * F * T), float(vis.numel() * 4)
+        link = {"h2d_gbs": b_in / t_in / 1e9, "d2h_gbs": b_out / t_out / 1e9,
+                "both_at_once_ms": t_both * 1e3, "both_at_once_gbs_total": (b_in + b_out) / t_both / 1e9,
+                "e2e_gbs_total": (b_in + b_out) / e2e_s / 1e9,
+                "note": "one monolithic pinned copy per direction; e2e interleaves channel-group copies in both directions"}
     checksum = int(vh.numpy()[0, :8, 0].astype(np.int64).sum())
 
     if rank != 0:
@@ -404,7 +428,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": "TOPS", "h2d_bytes_per_step": N * F * T,
                 "d2h_bytes_per_step": vis.numel() * 4, "ms_per_step": e2e_s * 1e3, "checksum": checksum,
                 "api": "corr_submit_host per step + corr_wait_host", "blocking_ms_per_step": e2e_blocking_s * 1e3,
-                "blocking_value": eff_ops(N, F, T) * world / e2e_blocking_s / 1e12},
+                "blocking_value": eff_ops(N, F, T) * world / e2e_blocking_s / 1e12, "link": link},
         "gpu_launches": args.steps * plan.info["kernels"],
         "roofline": roofline,
         "sustained": sustained,

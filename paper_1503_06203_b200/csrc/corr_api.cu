@@ -146,6 +146,7 @@ struct corr_plan {
     // dp4a only
     int aligned;
     // tcgen05 only
+    int pack_sub;      // variant 1: 128, or 64 when two 64-input channels are packed into one 128-tile (see below)
     int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh; chosen for N <= 128, where a pair tile would be
                        // half empty); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
                        // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
@@ -296,8 +297,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         else if (force && !strcmp(force, "imma"))
             path = CORR_PATH_IMMA;
         else
-            path = (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;   // both measured 3-10x the dp4a kernel
+            // N = 64 with an even number of channels: the stream [T][F][64] IS the stream [T][F/2][128], so a 128-tile
+            // holds two whole channels and its two diagonal 64-blocks are their matrices (half of the tensor work is
+            // cross-channel and dropped; still 1.45x the warp-MMA kernel, which is MMA-issue-bound at N = 64,
+            // profiles/r02_sweep.md)
+            path = (N == 64 && F % 2 == 0) ? CORR_PATH_TCGEN05 : (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;
     }
+    const bool packed64 = (path == CORR_PATH_TCGEN05 && N == 64 && F % 2 == 0);
     if (path == CORR_PATH_IMMA && n_pad > 64) {
         g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: the warp-MMA path takes N <= 64, got N=%d", N);
         return nullptr;
@@ -377,8 +383,11 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         // effective TOPS at N = 128, profiles/r02_sweep.md), so single-CTA tiles take over there
         const char *v = getenv("CORR_TC_VARIANT");   // testing aid: force a kernel
         p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "3")) ? 3 : (v && !strcmp(v, "5")) ? 5 : (n_pad <= 128) ? 1 : 3;
+        if (packed64) p->variant = 1;
     }
-    const int nb = (N + p->tile - 1) / p->tile;
+    p->pack_sub = packed64 ? 64 : 128;
+    const int Ns = packed64 ? 128 : N, Fs = packed64 ? F / 2 : F;   // the shape the tile schedule sees
+    const int nb = (Ns + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
     std::vector<ushort4> tiles4;
     if (p->variant >= 3) {
@@ -402,7 +411,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             for (int by = bx; by < nb; ++by) tiles.push_back(make_ushort2((unsigned short)bx, (unsigned short)by));
     }
     p->tiles_per_f = (int)tiles.size();
-    const long long units0 = (long long)F * p->tiles_per_f;
+    const long long units0 = (long long)Fs * p->tiles_per_f;
     if (units0 > 0x7fffffffLL / 64) {
         g_create_rc = CORR_ERR_INVALID_ARG; set_err("corr_plan_create: too many work units");
         delete p;
@@ -573,8 +582,10 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
         return CORR_OK;
     }
     // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
-    const cuuint64_t dims[3] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F, (cuuint64_t)p->T};
-    const cuuint64_t strides[2] = {(cuuint64_t)p->n_pad, (cuuint64_t)p->F * (cuuint64_t)p->n_pad};
+    // (two 64-input channels packed into one 128-tile: the same bytes seen as (128, F/2, T))
+    const cuuint64_t nw = (p->pack_sub == 64) ? 128 : (cuuint64_t)p->n_pad, fw = (p->pack_sub == 64) ? (cuuint64_t)p->F / 2 : (cuuint64_t)p->F;
+    const cuuint64_t dims[3] = {nw, fw, (cuuint64_t)p->T};
+    const cuuint64_t strides[2] = {nw, fw * nw};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const int st = (p->variant >= 3) ? corr::T3_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
@@ -685,8 +696,10 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
                 corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
         } else {
             corr::TcParams prm;
-            prm.N = p->N;
-            prm.F = p->F;
+            prm.N = (p->pack_sub == 64) ? 128 : p->N;
+            prm.F = (p->pack_sub == 64) ? p->F / 2 : p->F;
+            prm.sub = p->pack_sub;
+            prm.n_out = p->N;
             prm.T = p->T;
             prm.tiles_per_f = p->tiles_per_f;
             prm.slices = p->slices;

@@ -67,6 +67,9 @@ struct TcParams {
     int t_per_slice;   // multiple of TC_ST
     int num_units;     // F * tiles_per_f * slices
     int out_mode;      // OutMode
+    int sub;           // 128, or 64: the tile holds two whole channels of 64 inputs (N = 128, F = channels / 2); only the
+                       // two diagonal 64-blocks are written, as channels 2f and 2f + 1
+    int n_out;         // inputs per channel in the layout of vis
     const ushort2 *tiles;
     int32_t *vis;
 };
@@ -248,7 +251,9 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // ===================== S5: epilogue =====================
         const int q = warp & 3;  // TMEM lane quarter this warp may read
         uint8_t *stage = epi_g + (warp - TC_EPI_WARP0) * 32 * TC_EPI_PITCH;
-        const size_t Bn = (size_t)p.N * ((size_t)p.N + 1) / 2;
+        const size_t Bn = (size_t)p.n_out * ((size_t)p.n_out + 1) / 2;
+        const int cpt = TC_BLK / p.sub;   // channels per tile (1, or 2 when packed)
+        const int ssh = (p.sub == 64) ? 6 : 7;   // log2(sub)
         uint32_t acc_ph = 0;
         for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
             const int f = u / units_per_f, rem = u % units_per_f;
@@ -263,7 +268,7 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             for (int c = 0; c < 8; ++c) {
                 const int yc = y0 + c * 16;
                 // whole 32x16 block below the diagonal or outside the matrix: nothing to write
-                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N);
+                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N) || ((yc >> ssh) != (xw >> ssh));
                 if (!skip) {
                     uint32_t s1[16], rr[16], s2[16];
                     ptx::tmem_ld16(trow + c * 16, s1);
@@ -285,7 +290,8 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                         const int x = xw + rl;
                         if (x < p.N && y < p.N && x <= y) {
                             const int2 v = *reinterpret_cast<const int2 *>(stage + rl * TC_EPI_PITCH + col * 8);
-                            int32_t *o = p.vis + ((size_t)f * Bn + baseline_index(p.N, x, y)) * 2;
+                            const int cx = x >> ssh;     // packed: channel of the tile (same for x and y, see skip)
+                            int32_t *o = p.vis + ((size_t)(f * cpt + cx) * Bn + baseline_index(p.n_out, x - cx * p.sub, y - cx * p.sub)) * 2;
                             if (p.out_mode == OUT_STORE) {
                                 *reinterpret_cast<int2 *>(o) = v;
                             } else if (p.out_mode == OUT_RMW) {
