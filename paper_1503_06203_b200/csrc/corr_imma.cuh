@@ -1,12 +1,13 @@
 // corr_imma.cuh -- step S4' of the hot path for N = 16, 32, 48, 64: warp-level int8 tensor-core
 // MMA (mma.sync.m16n8k32.s8) on whole channels, fed by TMA.
 //
-// Why not dp4a here: measured on B200, IDP.4A issues 64 lanes/clk/SM = 17.5 T dp4a/s, i.e. 140
-// effective TOPS at one dp4a per complex MAC, while streaming N = 16 inputs at HBM speed needs
-// 4 (N + 1) ops per byte x 6.5 TB/s = 440 effective TOPS.  The legacy warp-level IMMA path
-// measures 1146 TOPS, enough to stay memory-bound up to N = 32.  Other N <= 64 run here on a stream
-// padded to the next multiple of 16 inputs (corr_pad_kernel below); corr_dp4a.cuh is only used on
-// request.  The paper makes the small-N observation for its own tiles at
+// Why not dp4a here: streaming N = 16 inputs at HBM speed needs 4 (N + 1) ops per byte x 6.5 TB/s = 440 effective
+// TOPS, and the CUDA-core kernel (one __dp4a per complex MAC, corr_dp4a.cuh) reached 0.37 TB/s on that shape where
+// this kernel reaches 4.2 - 4.7 (profiles/r01_sweep.csv, the dp4a figure in profiles/r01_sweep.md).  Warp-level
+// mma.sync keeps N = 16 and 32 memory-bound; at N = 48 and 64 it is bound by its own issue rate.  Other N <= 64 run
+// here on a stream padded to the next multiple of 16 inputs (corr_pad_kernel below); N = 64 with an even channel
+// count goes to single-CTA tcgen05 tiles instead (two channels per tile, corr_api.cu); corr_dp4a.cuh is only
+// used on request.  The paper makes the small-N observation for its own tiles at
 // PAPER.md:72; the result computed is Eq. 1 summed over time on the
 // upper triangle.
 //

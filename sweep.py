@@ -1,7 +1,7 @@
 """N sweep of the X-engine (the x-axis of the paper's Fig. 4) and the five BASELINE.json
 shapes: effective TOPS and achieved HBM GB/s per shape, device-timed with CUDA events.
 
-    python -m paper_1503_06203_b200.sweep [--reps 20] [--csv out.csv] [--shape N,F,T]
+    python sweep.py [--reps 20] [--csv out.csv] [--shape N,F,T] [--op corr|shift|gated]
 
 Inputs are random bytes generated on the device (every byte is a legal sample pair; timing does not
 depend on the values); correctness is the parity tests' job, not this script's.
@@ -10,6 +10,11 @@ from __future__ import annotations
 
 import argparse
 import sys
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
 
 # (label, N, F, T, accumulate): sweep shapes keep the input >= 256 MB for small N so GB/s means something
 SHAPES = [
@@ -26,7 +31,7 @@ def other_op(args):
     """Times corr_time_shift or corr_execute_gated on one shape (read + written bytes per second for the shift)."""
     import numpy as np
     import torch
-    from . import Plan, time_shift
+    from paper_1503_06203_b200 import Plan, time_shift
     n, f, t = (int(v) for v in (args.shape or "2048,8,8192").split(","))
     dev = torch.device("cuda:0")
     a = torch.randint(0, 256, (t, f, n), dtype=torch.uint8, device=dev)
@@ -67,7 +72,7 @@ def main():
         n, f, t = (int(v) for v in args.shape.split(","))
         shapes = [("shape", n, f, t, 0)]
     import torch
-    from . import Plan
+    from paper_1503_06203_b200 import Plan
     if not torch.cuda.is_available():
         sys.exit("sweep needs a CUDA device (there is no CPU path)")
     dev = torch.device("cuda:0")
