@@ -9,11 +9,10 @@
 //
 // HBM-bound gather: a CTA owns (channel, 128 inputs, SH_TB output samples); it loads the input rows
 // [t0 - max lag, t0 + SH_TB - min lag) of its 128 inputs into shared memory with 16-byte loads, then every
-// thread assembles 16 output bytes from the rows its inputs' lags select and writes them with one 16-byte
-// store (a single 16-byte shared-memory load when the 16 inputs share one lag, the common case of a few
-// cable lengths).  Read amplification (SH_TB + spread) / SH_TB, spread = max lag - min lag over the 128 inputs.  When
-// the spread does not fit, the CTA goes through its inputs 16 at a time with a 16-byte-wide window that can be
-// eight times longer (spreads up to 4480 samples); beyond that, or when N is not a multiple of 16, it gathers
+// thread assembles one 32-bit word of an output row from the rows its four inputs' lags select (a single 32-bit
+// shared-memory load when they share one lag) and a warp writes the 128-byte row.  Read amplification (SH_TB + spread) / SH_TB, spread = max lag - min lag over the 128 inputs.  When
+// the spread does not fit, one CTA in four goes through its inputs 16 at a time with a 16-byte-wide window that can be
+// eight times longer, for 512 output samples (spreads up to 4096 samples); beyond that, or when N is not a multiple of 16, it gathers
 // byte by byte from global memory (correct, slow).
 #pragma once
 #include <cstdint>
@@ -63,44 +62,41 @@ corr_shift_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, con
             *reinterpret_cast<uint4 *>(tile + r * 128 + 16 * c) = v;
         }
         __syncthreads();
-        // ---- assemble 16 output bytes per thread
-        // (SH_THREADS is a multiple of 8, so a thread keeps its column group c for every row it handles)
-        const int c = tid & 7;
-        bool same = true;
-        int off[16];   // shared-memory offset of this thread's 16 inputs relative to output row 0 (loop invariant)
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            same = same && (slag[16 * c + j] == slag[16 * c]);
-            off[j] = (hi - slag[16 * c + j]) * 128 + 16 * c + j;
-        }
-        if (c < c16n) {
-            for (int tr = tid >> 3; tr < tcount; tr += SH_THREADS / 8) {
-                uint4 v;
+        // ---- assemble one 32-bit word (4 inputs) per thread: a warp writes one output row of 128 bytes per step.
+        //      Lane l owns word l of the row whatever source row its lags select, and the staged rows are 128 bytes
+        //      = 32 banks apart, so the byte loads of a warp fall on 32 distinct banks (a thread that gathered 16
+        //      bytes met the other rows of its warp on the same banks: 4-way conflicts, profiles/r02_secondary_kernels.md)
+        const int wq = tid & 31;            // word of the row: inputs 4 wq .. 4 wq + 3
+        const int off0 = (hi - slag[4 * wq + 0]) * 128 + 4 * wq + 0, off1 = (hi - slag[4 * wq + 1]) * 128 + 4 * wq + 1;
+        const int off2 = (hi - slag[4 * wq + 2]) * 128 + 4 * wq + 2, off3 = (hi - slag[4 * wq + 3]) * 128 + 4 * wq + 3;
+        const bool same = (off1 == off0 + 1) && (off2 == off0 + 2) && (off3 == off0 + 3);   // the four inputs share a lag
+        if ((wq >> 2) < c16n) {
+            for (int tr = tid >> 5; tr < tcount; tr += SH_THREADS / 32) {
+                const uint8_t *rowp = tile + tr * 128;
+                uint32_t v;
                 if (same) {
-                    v = *reinterpret_cast<const uint4 *>(tile + tr * 128 + off[0]);
+                    v = *reinterpret_cast<const uint32_t *>(rowp + off0);
                 } else {
-                    const uint8_t *rowp = tile + tr * 128;
-                    uint32_t w[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const uint32_t b0 = rowp[off[4 * q + 0]], b1 = rowp[off[4 * q + 1]];
-                        const uint32_t b2 = rowp[off[4 * q + 2]], b3 = rowp[off[4 * q + 3]];
-                        w[q] = __byte_perm(b0 | (b1 << 8), b2 | (b3 << 8), 0x5410);
-                    }
-                    v = make_uint4(w[0], w[1], w[2], w[3]);
+                    const uint32_t b0 = rowp[off0], b1 = rowp[off1], b2 = rowp[off2], b3 = rowp[off3];
+                    v = __byte_perm(b0 | (b1 << 8), b2 | (b3 << 8), 0x5410);
                 }
-                *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) = v;
+                *reinterpret_cast<uint32_t *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 4 * wq) = v;
             }
         }
     } else if ((N & 15) == 0) {
-        // ---- wide spread: one group of 16 inputs at a time, so the window is 16 bytes wide and can be
-        //      8 x longer (spreads up to SH_MAX_ROWS * 8 - SH_TB rows inside a group of 16 inputs)
+        // ---- wide spread: one group of 16 inputs at a time, so the window is 16 bytes wide and can be 8 x longer.
+        //      Four consecutive CTAs along t share the work of one (the other three leave): 512 output rows per
+        //      window instead of 128 cut the re-read of the spread by four.  A thread assembles one 32-bit word;
+        //      a warp covers 8 rows x 4 words, which fall on 32 distinct banks (rows are 16 bytes = 4 banks apart).
+        if (blockIdx.z & 3) return;
+        const int tcw = min(4 * SH_TB, T - t0);
         const int c16n = ncols >> 4;
+        const int w = tid & 3, rl = tid >> 2;          // word of the group, row inside a block of 64 rows
         for (int c = 0; c < c16n; ++c) {
             int glo = 0x7fffffff, ghi = (int)0x80000000;
 #pragma unroll
             for (int j = 0; j < 16; ++j) { glo = min(glo, slag[16 * c + j]); ghi = max(ghi, slag[16 * c + j]); }
-            const long long grows = (long long)SH_TB + (long long)ghi - (long long)glo;
+            const long long grows = (long long)tcw + (long long)ghi - (long long)glo;
             if (grows <= SH_MAX_ROWS * 8) {
                 __syncthreads();   // the previous group's window is no longer read
                 for (int r = tid; r < (int)grows; r += SH_THREADS) {
@@ -111,23 +107,16 @@ corr_shift_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, con
                     *reinterpret_cast<uint4 *>(tile + r * 16) = v;
                 }
                 __syncthreads();
-                for (int tr = tid; tr < tcount; tr += SH_THREADS) {
-                    uint32_t w[4];
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        uint32_t acc = 0;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int n = 4 * q + j;
-                            acc |= (uint32_t)tile[(tr + ghi - slag[16 * c + n]) * 16 + n] << (8 * j);
-                        }
-                        w[q] = acc;
-                    }
-                    *reinterpret_cast<uint4 *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c) =
-                        make_uint4(w[0], w[1], w[2], w[3]);
+                const int o0 = (ghi - slag[16 * c + 4 * w + 0]) * 16 + 4 * w + 0, o1 = (ghi - slag[16 * c + 4 * w + 1]) * 16 + 4 * w + 1;
+                const int o2 = (ghi - slag[16 * c + 4 * w + 2]) * 16 + 4 * w + 2, o3 = (ghi - slag[16 * c + 4 * w + 3]) * 16 + 4 * w + 3;
+                for (int tr = rl; tr < tcw; tr += SH_THREADS / 4) {
+                    const uint8_t *rowp = tile + tr * 16;
+                    const uint32_t b0 = rowp[o0], b1 = rowp[o1], b2 = rowp[o2], b3 = rowp[o3];
+                    *reinterpret_cast<uint32_t *>(out + ((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + 16 * c + 4 * w) =
+                        __byte_perm(b0 | (b1 << 8), b2 | (b3 << 8), 0x5410);
                 }
             } else {
-                for (int idx = tid; idx < tcount * 16; idx += SH_THREADS) {
+                for (int idx = tid; idx < tcw * 16; idx += SH_THREADS) {
                     const int tr = idx >> 4, n = 16 * c + (idx & 15);
                     const long long tin = (long long)t0 + tr - slag[n];
                     uint8_t b = 0x88;
