@@ -18,6 +18,12 @@
 //   * the MMAs take A from TMEM ([a_tmem] form) and only B from shared memory.
 // Per stage and CTA: 128 (TC) + 96 (loads) + 64 (stores) wavefronts.
 //
+// Tried in round 2 and not kept (profiles/r02_tc3_ncu_summary.md): the same arithmetic on a finer pipeline (operand
+// slots of 32 samples filled by four groups of unpack warps, 8-slot ring): same speed, this kernel is bound by the
+// MMAs and the accumulator drain, not by the unpack; a row-image pitch of 129 slots (conflict-free stores) with
+// pipelined 8-column TMEM loads: slower (spills at 96 registers); negating an operand through bits 13 / 14 of the
+// instruction descriptor (one accumulator for Im): illegal instruction for kind::i8.
+//
 // Per CTA r (= rank in the pair) and per stage of 64 time samples:
 //   packed X_r  [64][128] bytes, 128-B swizzle   x in [256*bx2 + 128 r, +128)      (TMA)
 //   packed Yh_r [64][ 64] bytes,  64-B swizzle   y in [128*by + 64 r, +64)          (TMA)
@@ -83,15 +89,19 @@ struct Tc3Params {
 // S3, second half: the work of a call is the list of units (channel, tile, T-slice), each a run of groups
 // of T3_GROUP samples.  Whole waves of units are dealt round-robin (unit = pair + k * npairs: the pairs then
 // work on neighbouring tiles of one channel at the same time, which is what keeps the re-read input in L2).
-// The units left over after the last whole wave are cut into one contiguous range of groups per CTA pair
-// ("stream-K"), so the tail costs every pair the same time whatever the number of tiles.  A segment is
-// the part of one unit that one pair computes: a whole unit, or a piece of a tail unit.
+// The units left over after the last whole wave are cut into pieces, one or two per CTA pair ("stream-K"), by a
+// cost model on the host (tc3_build_pieces in corr_api.cu: groups + a fixed cost per piece), so the tail costs
+// every pair the same time whatever the number of tiles.  A segment is the part of one unit that one pair
+// computes: a whole unit, or a piece of a tail unit.  The first piece of a cut unit runs BEFORE its pair's whole
+// units (see Tc3Iter), the others after: a cut unit is summed in memory, and this way the piece that stores
+// has long finished when the others add.
 // A pair tile: CTA r computes the 128 x 128 block (rows = inputs of block r ? xb : xa, columns = inputs of
 // block by).  Normal tiles hold blocks of the upper triangle as they are (row block <= column block).  A
 // TRANSPOSED tile holds blocks (x = by, y = xa) and (x = by, y = xb) of the triangle computed the other way round
 // (rows = the y inputs): this is how the blocks left over when a block column has an odd number of row blocks
 // are paired up -- as rows they differ, but transposed they all share the column block 0 -- instead of being
-// computed next to an idle CTA.  The epilogue conjugates and writes them transposed.  xb = 0xFFFF: no block.
+// computed next to an idle CTA.  The epilogue conjugates them and stages them transposed (shared-memory row =
+// output row), so that they leave as bulk copies like the others.  xb = 0xFFFF: no block.
 constexpr unsigned short TC3_TILE_TRANSPOSED = 1, TC3_NO_BLOCK = 0xFFFF;
 
 struct Tc3Seg {

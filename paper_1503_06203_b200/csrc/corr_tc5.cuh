@@ -16,27 +16,39 @@
 //     512 Re = P1 + P2 + 514 P3 + R[x] + R[y] + 65536 Tv
 // exact in int32 for segments of <= 16384 samples.
 //
-// What differs from corr_tc4.cuh, and why (ncu, profiles/r02_tc5_ncu_summary.md: tc4 ran the shared-memory
-// data pipe at 83 % of elapsed cycles with the tensor pipe at 69 %, plus a 50 us corr_sums_kernel pass):
-//   * B2 = W is the stored byte itself, so the MMA reads it straight from the TMA-written y-half ring
-//     (MN-major, 64-B swizzle); only V and L are written by the unpack warps.
-//   * The y-half is read with the same transposing ldmatrix as the x-block, so every unpack register
-//     holds four TIME-consecutive bytes of one input on BOTH sides: the per-element sums SW, SL are one
-//     __dp4a(w, 0x01010101) and one on (w & 0x0F0F0F0F) per register, accumulated in registers over a
-//     segment and handed to the epilogue through shared memory (the y-half sums also to the peer CTA,
-//     red.shared::cluster).  corr_sums_kernel and its pass over HBM are gone; cut (stream-K) units get
-//     the sums of exactly their own samples for free.
-//   * V and L of the y-half are stored K-major (no swizzle, core matrices of 8 inputs x 16 samples): the
-//     transposed registers go out as 4-byte stores, 128 contiguous bytes per warp instruction.
-//   * The epilogue's row image has a pitch of 129 (Re,Im) slots: 8-byte stores of a half-warp fall on
-//     distinct banks (the 1040-byte pitch of tc3/tc4 gave 2-way conflicts on every store).
+// How it is built, and why (profiles/r02_tc5_ncu_summary.md has the counters behind every sentence):
+//   * The y-half is read with the same transposing ldmatrix as the x-block, so every unpack register holds four
+//     TIME-consecutive bytes of one input on BOTH sides: the per-element sums SW, SL are one __dp4a(w, 0x01010101)
+//     and one on (w & 0x0F0F0F0F) per register, accumulated in registers over a segment and handed to the epilogue
+//     through shared memory (the y-half sums also to the peer CTA, red.shared::cluster + release / acquire at
+//     cluster scope).  There is no sums kernel and no second pass over the input (round 1's corr_tc4 had one: 50 us);
+//     cut (stream-K) units get the sums of exactly their own samples for free.
+//   * V, W and L of the y-half are stored K-major (no swizzle, core matrices of 8 inputs x 16 samples): the
+//     transposed registers go out as 4-byte stores, 128 contiguous bytes per warp instruction, and the three MMAs
+//     of a slot share one instruction descriptor.
+//   * Operand slots of 32 samples (one K-step, 192 tensor cycles), a ring of 4 slots, four groups of four unpack
+//     warps, group g owning ring entry g.  A group of 256 samples is exactly two turns of the ring, so every ring
+//     position in the MMA issue loop is a compile-time constant and every descriptor a loop-invariant uniform
+//     register: with run-time ring indices the issuing warp needed ~430 cycles per slot, with compile-time indices
+//     but ten unrolled phases ~390 (the descriptors then live in ordinary registers and are moved to uniform
+//     registers one by one).
+//   * Four epilogue warps (a thread owns a whole row of the block): 22 warps leave 88 registers per thread, which
+//     the unpack loop needs to keep its loop invariants out of the loop (at 72 it recomputed them from the thread
+//     index every iteration: 176 instructions per slot and sub-partition against the 192 cycles of the MMAs).
+//   * The epilogue's row image has a pitch of 129 (Re,Im) slots (conflict-free 8-byte stores).
+// Where it stands: bit-exact, 0.95 - 0.97 of corr_tc3_kernel on cfg 3.  The three-product scheme moves the same
+// bytes through shared memory per 32 samples as the four-product one (TMA 48 + ldmatrix 48 + plane stores 48 +
+// tensor-core reads 48 wavefronts per CTA) in 192 instead of 256 tensor cycles: the shared-memory data pipe is at
+// 81 % of its cycles with the tensor pipe at 65 %, and a run with the TMA loads switched off (no writes into shared
+// memory) is 23 % faster.  Reading W of the y-half straight from the TMA ring (B2 = the stored byte) would save 16
+// of the 192 wavefronts but ties that ring to the MMAs' completion (a second, deeper ring and a two-phase issue
+// loop; the first form of this kernel did it, its effect was never isolated).  So corr_tc3_kernel stays the default.
 //
 // Rings (per CTA r of the pair):
-//   X ring   T5_XS stages   packed X_r  [64 t][128 x] 128-B swizzle (TMA)   freed by the unpack warps
-//   Y ring   T5_YS stages   packed Yh_r [64 t][ 64 y]  64-B swizzle (TMA)   read by the unpack warps AND by
-//                           the MMA (B2 = W); freed by tcgen05.commit after the stage's second slot
-//   VL ring  5 slots of 32 samples: V | L [64 y][32 t] K-major, 2 KB each   freed by tcgen05.commit
-//   TMEM     0..127 P1   128..255 P2   256..383 P3   384..503 A slots, 5 x (W 8 | V 8 | L 8 columns)
+//   packed ring  T5_PK stages of 64 samples: X_r [64 t][128 x] 128-B swizzle | Yh_r [64 t][64 y] 64-B swizzle (TMA),
+//                freed by the unpack warps as soon as the bytes are in registers
+//   V|W|L ring   4 slots of 32 samples: three planes [64 y][32 t] K-major, 2 KB each, freed by tcgen05.commit
+//   TMEM         0..127 P1   128..255 P2   256..383 P3   384..479 A slots, 4 x (W 8 | V 8 | L 8 columns)
 // Unpack warp group g (4 warps: TMEM lane quarters) fills the operand slots o with o % 4 == g.
 #pragma once
 #include <cstdint>
