@@ -37,9 +37,23 @@ def other_op(args):
     a = torch.randint(0, 256, (t, f, n), dtype=torch.uint8, device=dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if args.op == "shift":
-        lags = torch.randint(-16, 17, (n,), dtype=torch.int32, device=dev)
+        # three lag patterns: every input its own lag, 16 inputs sharing a lag (a few cable lengths), a wide spread
         out = torch.empty_like(a)
-        run = lambda: time_shift(a, lags, out=out)
+        pats = {"independent +-16": torch.randint(-16, 17, (n,), dtype=torch.int32, device=dev),
+                "shared by 16 inputs +-16": torch.randint(-16, 17, ((n + 15) // 16,), dtype=torch.int32, device=dev).repeat_interleave(16)[:n].contiguous(),
+                "independent +-256": torch.randint(-256, 257, (n,), dtype=torch.int32, device=dev)}
+        for name, lags in pats.items():
+            for _ in range(3):
+                time_shift(a, lags, out=out)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(args.reps):
+                time_shift(a, lags, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.reps
+            print(f"shift,{name},N={n},F={f},T={t},ms={ms:.4g},read+written_GBs={2 * a.numel() / (ms * 1e-3) / 1e9:.4g}")
+        return
     else:
         plan = Plan(n, f, t)
         gate = ((np.arange(t) % 64) * 4 // 64).astype(np.int32)
