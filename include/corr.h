@@ -185,6 +185,19 @@ int corr_plan_info(const corr_plan *plan, int info[8]);
  * (host only; the scheduler's counting rule, Fig. 1: N=256, 32x32 -> 36). */
 int corr_count_tiles(int N, int tile_x, int tile_y);
 
+/* The schedule of the CTA-pair kernels (step S3; PAPER.md:64-72 for the triangular tiling, PAPER.md:21 for channels as
+ * independent work) for a problem (N, F, T) on `pairs` CTA pairs, computed without a device by the same code
+ * corr_plan_create runs (host only).  A unit is (channel, pair tile, T-slice) = groups of 256 samples; whole waves of
+ * units are dealt round-robin (unit = pair + k * pairs), the units left over are cut into pieces.
+ *   info[0] pair tiles per channel        info[1] T-slices                info[2] units
+ *   info[3] groups per full slice         info[4] groups in the last slice of a tile
+ *   info[5] CTA pairs used (<= pairs)     info[6] whole waves             info[7] transposed tiles per channel
+ *   pieces  NULL, or caller-owned int[pairs][4][4]: for every used pair up to 4 pieces (unit, first group, number of
+ *           groups, early); entries with 0 groups are unused.  early = 1: the piece is computed before the pair's
+ *           whole units (it is the first piece of a cut unit and stores; the others add).
+ * Returns CORR_OK or CORR_ERR_INVALID_ARG. */
+int corr_schedule_pairs(int N, int F, int T, int pairs, int info[8], int *pieces);
+
 #ifdef __cplusplus
 }
 #endif

@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops", "corr_submit_host", "corr_wait_host")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_schedule_pairs", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops", "corr_submit_host", "corr_wait_host")
 
 
 class CorrError(RuntimeError):
@@ -61,6 +61,8 @@ def load_library():
         lib.corr_plan_info.restype = ci
         lib.corr_count_tiles.argtypes = [ci, ci, ci]
         lib.corr_count_tiles.restype = ci
+        lib.corr_schedule_pairs.argtypes = [ci, ci, ci, ci, ctypes.POINTER(ci * 8), vp]
+        lib.corr_schedule_pairs.restype = ci
         lib.corr_execute_gated.argtypes = [vp, vp, vp, ci, vp, ci, vp]
         lib.corr_execute_gated.restype = ci
         lib.corr_measure_int8_tops.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
@@ -160,6 +162,21 @@ def baseline_index(N: int, x: int, y: int) -> int:
 
 def count_tiles(N: int, tile_x: int, tile_y: int) -> int:
     return int(load_library().corr_count_tiles(N, tile_x, tile_y))
+
+
+def schedule_pairs(N: int, F: int, T: int, pairs: int):
+    """corr_schedule_pairs: (info dict, pieces) with pieces[pair] = list of (unit, first group, groups, early)."""
+    lib = load_library()
+    info = (ctypes.c_int * 8)()
+    buf = (ctypes.c_int * (16 * pairs))()
+    rc = lib.corr_schedule_pairs(N, F, T, pairs, ctypes.byref(info), ctypes.cast(buf, ctypes.c_void_p))
+    if rc != 0:
+        raise CorrError(f"corr_schedule_pairs -> {rc}: {_err()}")
+    keys = ("tiles_per_channel", "slices", "units", "groups_full", "groups_last", "pairs_used", "waves", "transposed_tiles")
+    d = dict(zip(keys, (int(v) for v in info)))
+    pieces = [[tuple(buf[16 * p + 4 * k + j] for j in range(4)) for k in range(4) if buf[16 * p + 4 * k + 2] > 0]
+              for p in range(d["pairs_used"])]
+    return d, pieces
 
 
 # ------------------------------------------------------------------ convenience wrapper

@@ -126,6 +126,26 @@ static void tc3_build_pieces(int num_units, int npairs, int slices, int groups_f
     assign(hi, true);
 }
 
+// S3, the tile table of the CTA-pair kernels (corr_tc3.cuh): pair tiles of two row blocks (128 inputs each) against
+// one column block.  Column block j needs the row blocks 0..j.  An even count pairs up as (0,1), (2,3), ...; an odd
+// count as (1,2), (3,4), ... and leaves block (0, j) over.  The left-over blocks all have row block 0: computed
+// transposed (rows = block j, columns = block 0) they share their column operand, so they pair up with each other.
+static void tc3_tile_table(int N, std::vector<ushort4> &tiles4)
+{
+    const int nb = (N + 127) / 128;
+    auto us = [](int v) { return (unsigned short)v; };
+    std::vector<int> left;
+    tiles4.clear();
+    for (int j = 0; j < nb; ++j) {
+        const int first = ((j + 1) % 2 == 0) ? 0 : 1;
+        for (int a = first; a + 1 <= j; a += 2) tiles4.push_back(make_ushort4(us(a), us(a + 1), us(j), 0));
+        if (first == 1) left.push_back(j);
+    }
+    for (size_t i = 0; i < left.size(); i += 2)
+        tiles4.push_back(make_ushort4(us(left[i]), (i + 1 < left.size()) ? us(left[i + 1]) : corr::TC3_NO_BLOCK, 0,
+                                      corr::TC3_TILE_TRANSPOSED));
+}
+
 static bool alloc_pad_buf(struct corr_plan *p);
 
 struct corr_plan {
@@ -203,6 +223,39 @@ size_t corr_baseline_index(int N, int x, int y)
 }
 
 int corr_count_tiles(int N, int tile_x, int tile_y) { return count_tiles(N, tile_x, tile_y); }
+
+int corr_schedule_pairs(int N, int F, int T, int pairs, int info[8], int *pieces_out)
+{
+    if (N < 1 || F < 1 || T < 1 || T > 16777215 || pairs < 1 || !info) {
+        set_err("corr_schedule_pairs: need N, F, pairs >= 1, 1 <= T <= 16777215 and an info array");
+        return CORR_ERR_INVALID_ARG;
+    }
+    std::vector<ushort4> tiles4;
+    tc3_tile_table(N, tiles4);
+    const long long units0 = (long long)F * (long long)tiles4.size();
+    if (units0 > 0x7fffffffLL / 64) {
+        set_err("corr_schedule_pairs: too many work units");
+        return CORR_ERR_INVALID_ARG;
+    }
+    const int Q = corr::T3_GROUP, s = (T + corr::TC_MAX_SLICE - 1) / corr::TC_MAX_SLICE;
+    const int tps = ((T + s - 1) / s + Q - 1) / Q * Q, slices = (T + tps - 1) / tps;
+    const int num_units = (int)(units0 * slices);
+    const int groups_full = tps / Q, groups_last = (T - (slices - 1) * tps + Q - 1) / Q;
+    const long long total_groups = units0 * ((long long)(slices - 1) * groups_full + groups_last);
+    const int used = (int)std::min<long long>(total_groups, pairs);
+    info[0] = (int)tiles4.size(); info[1] = slices; info[2] = num_units; info[3] = groups_full; info[4] = groups_last;
+    info[5] = used; info[6] = num_units / used; info[7] = 0;
+    for (const ushort4 &t : tiles4) info[7] += (t.w & corr::TC3_TILE_TRANSPOSED) ? 1 : 0;
+    if (pieces_out) {
+        std::vector<int4> pieces;
+        tc3_build_pieces(num_units, used, slices, groups_full, groups_last, tiles4, pieces);
+        for (size_t i = 0; i < pieces.size(); ++i) {
+            pieces_out[4 * i + 0] = pieces[i].x; pieces_out[4 * i + 1] = pieces[i].y;
+            pieces_out[4 * i + 2] = pieces[i].z; pieces_out[4 * i + 3] = pieces[i].w;
+        }
+    }
+    return CORR_OK;
+}
 
 size_t corr_input_bytes(const corr_plan *p) { return p ? (size_t)p->T * p->F * p->N : 0; }
 
@@ -391,20 +444,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     std::vector<ushort2> tiles;
     std::vector<ushort4> tiles4;
     if (p->variant >= 3) {
-        // Pair tiles of two row blocks (128 inputs each) against one column block.  Column block j needs the row
-        // blocks 0..j.  An even count pairs up as (0,1), (2,3), ...; an odd count as (1,2), (3,4), ... and leaves
-        // block (0, j) over.  The left-over blocks all have row block 0: computed transposed (rows = block j,
-        // columns = block 0) they share their column operand, so they pair up with each other.
-        auto us = [](int v) { return (unsigned short)v; };
-        std::vector<int> left;
-        for (int j = 0; j < nb; ++j) {
-            const int first = ((j + 1) % 2 == 0) ? 0 : 1;
-            for (int a = first; a + 1 <= j; a += 2) tiles4.push_back(make_ushort4(us(a), us(a + 1), us(j), 0));
-            if (first == 1) left.push_back(j);
-        }
-        for (size_t i = 0; i < left.size(); i += 2)
-            tiles4.push_back(make_ushort4(us(left[i]), (i + 1 < left.size()) ? us(left[i + 1]) : corr::TC3_NO_BLOCK, 0,
-                                          corr::TC3_TILE_TRANSPOSED));
+        tc3_tile_table(Ns, tiles4);
         tiles.resize(tiles4.size());   // the count is what the schedule below needs
     } else {
         for (int bx = 0; bx < nb; ++bx)

@@ -180,6 +180,25 @@ def test_determinism(corr):
     assert np.array_equal(_run(corr, packed, corr.PATH_IMMA)[0], _run(corr, packed, corr.PATH_TCGEN05)[0])
 
 
+@pytest.mark.parametrize("F", [2, 6, 16, 3])
+def test_n64_two_channels_per_tile(corr, oracle, F):
+    # N = 64, even F: AUTO runs single-CTA tcgen05 tiles on the stream seen as [T][F/2][128] and writes the two
+    # diagonal 64-blocks of each tile as channels 2f, 2f + 1; odd F stays on the warp-MMA kernel.  Ragged T, split T,
+    # stale output, accumulation, extreme bytes.
+    for T in (1, 63, 300, 4099, 70000 if F == 2 else 1000):
+        packed = workloads.uniform_bytes(64, F, T, seed=64 * F + T)
+        want = oracle.level1(packed)
+        got, info = _run(corr, packed, corr.PATH_AUTO, prefill=-559038737)
+        assert info["path"] == (corr.PATH_TCGEN05 if F % 2 == 0 else corr.PATH_IMMA)
+        assert np.array_equal(got, want), (F, T)
+        again, _ = _run(corr, packed, corr.PATH_AUTO, accumulate_into=got.copy())
+        assert np.array_equal(again, 2 * want), (F, T, "accumulate")
+    for byte in (0x00, 0xFF):
+        packed = np.full((2048, F, 64), byte, np.uint8)
+        got, _ = _run(corr, packed, corr.PATH_AUTO)
+        assert np.array_equal(got, oracle.level1(packed)), (F, hex(byte))
+
+
 @pytest.mark.parametrize("variant", ["1", "3", "5"])
 def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
     # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles (automatic for N <= 128), 3 CTA pair
