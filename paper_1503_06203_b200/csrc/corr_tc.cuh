@@ -268,7 +268,7 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             for (int c = 0; c < 8; ++c) {
                 const int yc = y0 + c * 16;
                 // whole 32x16 block below the diagonal or outside the matrix: nothing to write
-                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N) || ((yc >> ssh) != (xw >> ssh));
+                const bool skip = (yc + 15 < xw) || (yc >= p.N) || (xw >= p.N) || (((yc - y0) >> ssh) != ((xw - x0) >> ssh));   // packed: the other channel's columns
                 if (!skip) {
                     uint32_t s1[16], rr[16], s2[16];
                     ptx::tmem_ld16(trow + c * 16, s1);
@@ -290,7 +290,7 @@ corr_tc_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                         const int x = xw + rl;
                         if (x < p.N && y < p.N && x <= y) {
                             const int2 v = *reinterpret_cast<const int2 *>(stage + rl * TC_EPI_PITCH + col * 8);
-                            const int cx = x >> ssh;     // packed: channel of the tile (same for x and y, see skip)
+                            const int cx = (x - x0) >> ssh;   // packed: channel of the tile (same for x and y, see skip)
                             int32_t *o = p.vis + ((size_t)(f * cpt + cx) * Bn + baseline_index(p.n_out, x - cx * p.sub, y - cx * p.sub)) * 2;
                             if (p.out_mode == OUT_STORE) {
                                 *reinterpret_cast<int2 *>(o) = v;
