@@ -40,9 +40,10 @@
 // bytes through shared memory per 32 samples as the four-product one (TMA 48 + ldmatrix 48 + plane stores 48 +
 // tensor-core reads 48 wavefronts per CTA) in 192 instead of 256 tensor cycles: the shared-memory data pipe is at
 // 81 % of its cycles with the tensor pipe at 65 %, and a run with the TMA loads switched off (no writes into shared
-// memory) is 23 % faster.  Reading W of the y-half straight from the TMA ring (B2 = the stored byte) would save 16
-// of the 192 wavefronts but ties that ring to the MMAs' completion (a second, deeper ring and a two-phase issue
-// loop; the first form of this kernel did it, its effect was never isolated).  So corr_tc3_kernel stays the default.
+// memory) is 23 % faster.  Reading W of the y-half straight from the TMA ring (B2 = the stored byte, MN-major) saves
+// 16 of the 192 wavefronts but ties that ring to the MMAs' completion (its own 8-stage ring, a two-phase issue loop,
+// two instruction descriptors per slot): built on this same kernel and measured, 333 against 306 us.  So W is stored
+// like V and L, and corr_tc3_kernel stays the default.
 //
 // Rings (per CTA r of the pair):
 //   packed ring  T5_PK stages of 64 samples: X_r [64 t][128 x] 128-B swizzle | Yh_r [64 t][64 y] 64-B swizzle (TMA),
