@@ -592,12 +592,40 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
         set_err("corr_time_shift: buffers must be 16-byte aligned");
         return CORR_ERR_INVALID_ARG;
     }
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (N % 16 != 0 || (N + 127) / 128 > corr::SH_MAX_GROUPS) {
+        dim3 grid((unsigned)((N + 127) / 128), (unsigned)F, (unsigned)((T + corr::SH_TB - 1) / corr::SH_TB));
+        corr::corr_shift_bytes_kernel<<<grid, 256, 0, stream>>>(packed_in_dev, packed_out_dev, lags_dev, N, F, T);
+        CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+        return CORR_OK;
+    }
+    if (!get_encode_fn()) {
+        set_err("corr_time_shift: cuTensorMapEncodeTiled not available from the driver");
+        return CORR_ERR_CUDA;
+    }
+    // the input as a 3-D byte tensor, innermost first: (N, F, T); a box is 16 rows of 128 inputs of one channel
+    CUtensorMap tmap;
+    const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)F, (cuuint64_t)T};
+    const cuuint64_t strides[2] = {(cuuint64_t)N, (cuuint64_t)F * (cuuint64_t)N};
+    const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)corr::SH_BOX_ROWS};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    CUresult r = get_encode_fn()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_in_dev), dims, strides,
+                                 box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_err("corr_time_shift: cuTensorMapEncodeTiled failed with CUresult %d (N=%d F=%d T=%d)", (int)r, N, F, T);
+        return CORR_ERR_CUDA;
+    }
+    int dev = 0, sms = 0;
+    CUDA_TRY(cudaGetDevice(&dev), CORR_ERR_CUDA);
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), CORR_ERR_CUDA);
     // the attribute belongs to the current device's context: set it on every call (a host-side table write)
     CUDA_TRY(cudaFuncSetAttribute(corr::corr_shift_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::SH_SMEM_BYTES),
              CORR_ERR_CUDA);
-    dim3 grid((unsigned)((N + 127) / 128), (unsigned)F, (unsigned)((T + corr::SH_TB - 1) / corr::SH_TB));
-    corr::corr_shift_kernel<<<grid, corr::SH_THREADS, corr::SH_SMEM_BYTES, static_cast<cudaStream_t>(stream_)>>>(
-        packed_in_dev, packed_out_dev, lags_dev, N, F, T);
+    const long long tiles = (long long)((N + 127) / 128) * F * ((T + corr::SH_TB - 1) / corr::SH_TB);
+    const unsigned grid = (unsigned)std::min<long long>(tiles, sms);
+    corr::corr_shift_kernel<<<grid, corr::SH_THREADS, corr::SH_SMEM_BYTES, stream>>>(tmap, packed_in_dev, packed_out_dev, lags_dev,
+                                                                                   N, F, T);
     CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
     return CORR_OK;
 }

@@ -86,6 +86,35 @@ def test_time_shift_parity(corr, oracle):
 
 
 @pytest.mark.gpu
+def test_time_shift_long_stream_mixed_spreads(corr, oracle):
+    # every group of 128 inputs takes its own route through the kernel (windows of one and of two time blocks, the
+    # 16-byte-wide window, byte by byte), over enough tiles per CTA to wrap the ring of rows several times
+    rng = np.random.default_rng(29)
+    T, F, N = 40000, 2, 5 * 128 + 48
+    packed = rng.integers(0, 256, (T, F, N), dtype=np.uint8)
+    lags = np.zeros(N, np.int64)
+    lags[0:128] = rng.integers(-8, 9, 128)
+    lags[128:256] = 1000 + rng.integers(-90, 91, 128)        # a common offset costs nothing: only the spread counts
+    lags[256:384] = rng.integers(-450, 451, 128)
+    lags[384:512] = rng.integers(-1900, 1901, 128)
+    lags[512:640] = rng.integers(-30000, 30001, 128)
+    lags[640:] = -7
+    assert np.array_equal(_gpu_shift(corr, packed, lags), oracle.time_shift(packed, lags))
+
+
+@pytest.mark.gpu
+def test_time_shift_many_tiles_per_cta(corr, oracle):
+    # one group of inputs, one channel: every CTA walks two dozen tiles whose windows (128 + 32 rows) fill the ring of
+    # rows exactly, so the ring wraps at its last row
+    rng = np.random.default_rng(31)
+    T, F, N = 128 * 148 * 24 + 77, 1, 128
+    packed = rng.integers(0, 256, (T, F, N), dtype=np.uint8)
+    lags = rng.integers(-16, 17, N)
+    lags[5], lags[77] = -16, 16
+    assert np.array_equal(_gpu_shift(corr, packed, lags), oracle.time_shift(packed, lags))
+
+
+@pytest.mark.gpu
 def test_time_shift_then_correlate(corr, oracle):
     # the two kernels chained on the device give what the oracle gives for the same chain
     import torch
