@@ -123,9 +123,11 @@ int corr_execute_host(corr_plan *plan, const uint8_t *packed_host, int32_t *vis_
  *   G           number of gates, >= 1 (at most T distinct run lengths are planned and cached)
  *   vis_dev     DEVICE pointer, G*F*N(N+1)/2*2 int32, layout [G][F][B][2]
  *   accumulate_flag  as for corr_execute, applied to every gate (a gate with no sample is zeroed / left)
- * Enqueues on `stream` (a row gather into plan-owned scratch, then one ordinary pass per gate); may
- * wait for the previous gated call's index upload; the first call with a new run length creates a
- * plan for it.  Returns CORR_OK or an error code. */
+ * Enqueues on `stream` (a row gather into plan-owned scratch, then ONE ordinary pass over all gates as G*F
+ * channels when the gates hold about the same number of samples -- the longest at most 5/4 of the mean, shorter
+ * ones filled up with stored zeros -- else one pass per gate; environment CORR_GATED_PER_GATE forces the
+ * latter); may wait for the previous gated call's index upload; the first call with a new run length creates
+ * a plan for it.  Returns CORR_OK or an error code. */
 int corr_execute_gated(corr_plan *plan, const uint8_t *packed_dev, const int32_t *gate_host, int G,
                        int32_t *vis_dev, int accumulate_flag, corr_stream_t stream);
 

@@ -188,11 +188,12 @@ struct corr_plan {
     unsigned long long grp_seq;   // channel groups submitted so far (staging buffers alternate across calls)
     unsigned long long calls_submitted;
     // corr_execute_gated: per-gate runs of the gathered stream, plans for their lengths
-    uint8_t *gate_buf;     // device, T*F*N bytes: rows regrouped by gate
-    int *order_dev;        // device, T row indices
+    uint8_t *gate_buf;     // device: rows regrouped by gate
+    size_t gate_buf_bytes;
+    int *order_dev;        // device, T row indices, then the (start, count) of every gate (at most GATE_MERGE_MAX_G)
     int *order_pin;        // pinned host copy the upload reads from
     cudaEvent_t ev_gate;   // the upload of order_pin has been consumed
-    std::map<int, corr_plan *> *gate_plans;   // length of a run -> plan (N, F, length)
+    std::map<long long, corr_plan *> *gate_plans;   // length of a run -> plan (N, F, length); (G << 32 | length) -> plan (N, G*F, length)
 };
 
 extern "C" void corr_plan_destroy(corr_plan *p);
@@ -783,6 +784,8 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     return CORR_OK;
 }
 
+constexpr int GATE_MERGE_MAX_G = 1024;   // gates that can share one pass (their starts and counts travel with the row order)
+
 int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *gate_host, int G, int32_t *vis_dev,
                        int accumulate_flag, corr_stream_t stream_)
 {
@@ -813,11 +816,14 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
         int *pin = nullptr, *odev = nullptr;
         uint8_t *gbuf = nullptr;
         cudaEvent_t ev = nullptr;
-        const bool ok = cudaMallocHost(&pin, (size_t)T * sizeof(int)) == cudaSuccess &&
+        // rows of all gates + alignment padding per run; or the gates side by side, padded to the longest (<= 5/4)
+        const size_t gbytes = std::max((size_t)T * row_bytes + 16 * (size_t)T + 16, ((size_t)T + (size_t)T / 4 + 1) * row_bytes);
+        const size_t oints = (size_t)T + 2 * (size_t)GATE_MERGE_MAX_G;
+        const bool ok = cudaMallocHost(&pin, oints * sizeof(int)) == cudaSuccess &&
                         cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess &&
-                        cudaMalloc(&odev, (size_t)T * sizeof(int)) == cudaSuccess &&
-                        cudaMalloc(&gbuf, (size_t)T * row_bytes + 16 * (size_t)T + 16) == cudaSuccess;   // + alignment padding per run
-        std::map<int, corr_plan *> *plans = ok ? new (std::nothrow) std::map<int, corr_plan *>() : nullptr;
+                        cudaMalloc(&odev, oints * sizeof(int)) == cudaSuccess &&
+                        cudaMalloc(&gbuf, gbytes) == cudaSuccess;
+        std::map<long long, corr_plan *> *plans = ok ? new (std::nothrow) std::map<long long, corr_plan *>() : nullptr;
         if (!ok || !plans) {
             set_err("corr_execute_gated: allocation of the gating scratch failed: %s", cudaGetErrorString(cudaGetLastError()));
             if (gbuf) cudaFree(gbuf);
@@ -829,6 +835,7 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
         p->ev_gate = ev;
         p->order_dev = odev;
         p->gate_buf = gbuf;
+        p->gate_buf_bytes = gbytes;
         p->gate_plans = plans;
         p->order_pin = pin;
     } else {
@@ -842,6 +849,39 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
             if (gate_host[t] >= 0) p->order_pin[fill[(size_t)gate_host[t]]++] = t;
     }
     const int used = start[(size_t)G];
+    // ---- gates of about the same length (a periodic signal cut into G phase bins): ONE pass over all of them.  The
+    //      gathered rows are laid out [j][g][F][N] (sample j of gate g; gates shorter than the longest are filled up
+    //      with stored zeros, which add nothing), which is the stream of G*F channels and max-length samples, and
+    //      its visibilities [G*F][B] are vis[G][F][B]: G times fewer launches, cold starts and tails
+    const int tmax = *std::max_element(count.begin(), count.end());
+    if (G >= 2 && G <= GATE_MERGE_MAX_G && row_bytes % 16 == 0 && used > 0 && (long long)G * p->F <= 65535 &&
+        (long long)tmax * G <= (long long)used + used / 4 && (size_t)tmax * G * row_bytes <= p->gate_buf_bytes &&
+        !getenv("CORR_GATED_PER_GATE")) {
+        const long long key = ((long long)G << 32) | (long long)tmax;
+        auto it = p->gate_plans->find(key);
+        if (it == p->gate_plans->end()) {
+            if (p->gate_plans->size() >= 64) {
+                corr_plan_destroy(p->gate_plans->begin()->second);   // waits for its kernels (cudaFree inside)
+                p->gate_plans->erase(p->gate_plans->begin());
+            }
+            corr_plan *np = corr_plan_create_ex(p->N, G * p->F, tmax, p->path);
+            if (!np) return g_create_rc;
+            it = p->gate_plans->emplace(key, np).first;
+        }
+        for (int g = 0; g < G; ++g) {
+            p->order_pin[(size_t)T + 2 * (size_t)g] = start[(size_t)g];
+            p->order_pin[(size_t)T + 2 * (size_t)g + 1] = count[(size_t)g];
+        }
+        CUDA_TRY(cudaMemcpyAsync(p->order_dev, p->order_pin, (size_t)used * sizeof(int), cudaMemcpyHostToDevice, stream),
+                 CORR_ERR_CUDA);
+        CUDA_TRY(cudaMemcpyAsync(p->order_dev + T, p->order_pin + T, 2 * (size_t)G * sizeof(int), cudaMemcpyHostToDevice, stream),
+                 CORR_ERR_CUDA);
+        CUDA_TRY(cudaEventRecord(p->ev_gate, stream), CORR_ERR_CUDA);
+        corr::corr_gate_gather_merged_kernel<<<8 * p->sm_count, corr::GATE_THREADS, 0, stream>>>(
+            packed_dev, p->gate_buf, p->order_dev, reinterpret_cast<const int2 *>(p->order_dev + T), G, tmax, (int)(row_bytes / 16));
+        CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+        return corr_execute(it->second, p->gate_buf, vis_dev, accumulate_flag, stream_);
+    }
     // byte offset of every gate's run in gate_buf: runs start on 16-byte boundaries (corr_execute needs that)
     std::vector<size_t> off((size_t)G, 0);
     {
@@ -877,13 +917,13 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
             if (!accumulate_flag) CUDA_TRY(cudaMemsetAsync(vis_g, 0, vis_per_gate * sizeof(int32_t), stream), CORR_ERR_CUDA);
             continue;
         }
-        auto it = p->gate_plans->find(len);
+        auto it = p->gate_plans->find((long long)len);
         if (it == p->gate_plans->end()) {
             if (p->gate_plans->size() >= 64) {
                 // bound the cache: drop ONE plan whose run length this call does not use (its kernels, if any are
                 // still in flight from an earlier call, are waited for by the cudaFree inside destroy)
                 for (auto ev = p->gate_plans->begin(); ev != p->gate_plans->end(); ++ev)
-                    if (std::find(count.begin(), count.end(), ev->first) == count.end()) {
+                    if ((ev->first >> 32) != 0 || std::find(count.begin(), count.end(), (int)ev->first) == count.end()) {
                         corr_plan_destroy(ev->second);
                         p->gate_plans->erase(ev);
                         break;
@@ -891,7 +931,7 @@ int corr_execute_gated(corr_plan *p, const uint8_t *packed_dev, const int32_t *g
             }
             corr_plan *np = corr_plan_create_ex(p->N, p->F, len, p->path);
             if (!np) return g_create_rc;   // the sub-plan's own error (message already set)
-            it = p->gate_plans->emplace(len, np).first;
+            it = p->gate_plans->emplace((long long)len, np).first;
         }
         int rc = corr_execute(it->second, p->gate_buf + off[(size_t)g], vis_g, accumulate_flag, stream_);
         if (rc != CORR_OK) return rc;

@@ -30,6 +30,24 @@ corr_gate_gather_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ ou
     }
 }
 
+// the gates side by side: out row j * G + g = in row order[gates[g].x + j] for j < gates[g].y (the gate's count), else a
+// row of stored zeros (0x88: the sample 0 + 0i); j < tmax
+__global__ void __launch_bounds__(GATE_THREADS)
+corr_gate_gather_merged_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out, const int *__restrict__ order,
+                               const int2 *__restrict__ gates, int G, int tmax, int row_vecs)
+{
+    const long long total = (long long)tmax * G * row_vecs;
+    for (long long i = (long long)blockIdx.x * GATE_THREADS + threadIdx.x; i < total;
+         i += (long long)gridDim.x * GATE_THREADS) {
+        const long long r = i / row_vecs;
+        const int v = (int)(i - r * row_vecs), j = (int)(r / G), g = (int)(r - (long long)j * G);
+        const int2 sc = __ldg(gates + g);
+        uint4 w = make_uint4(0x88888888u, 0x88888888u, 0x88888888u, 0x88888888u);
+        if (j < sc.y) w = __ldg(reinterpret_cast<const uint4 *>(in) + (size_t)__ldg(order + sc.x + j) * row_vecs + v);
+        reinterpret_cast<uint4 *>(out)[i] = w;
+    }
+}
+
 // same for rows that are not a multiple of 16 bytes
 __global__ void __launch_bounds__(GATE_THREADS)
 corr_gate_gather_bytes_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ out,

@@ -73,9 +73,13 @@ def corr():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("per_gate", [False, True])
 @pytest.mark.parametrize("shape", [(16, 5, 3000), (64, 3, 2500), (100, 2, 900), (272, 2, 2000), (1024, 1, 1500)])
-def test_gated_parity(corr, oracle, shape):
+def test_gated_parity(corr, oracle, shape, per_gate, monkeypatch):
+    # gates of about the same length share one pass (the gates as extra channels); per_gate forces one pass per gate
     import torch
+    if per_gate:
+        monkeypatch.setenv("CORR_GATED_PER_GATE", "1")
     N, F, T = shape
     packed = workloads.iid_gaussian(N, F, T, seed=N + T)
     dev = torch.from_numpy(packed).cuda()
