@@ -141,7 +141,8 @@ int corr_execute_gated(corr_plan *plan, const uint8_t *packed_dev, const int32_t
  *                                  distinct, 16-byte aligned when N % 16 == 0; caller-owned
  *   lags_dev                       DEVICE pointer, N int32 (any values; |lag| >= T empties the element)
  * N % 16 == 0 and N <= 65536 take the TMA-fed kernel (a tensor map of the input is encoded per call, on the
- * host); other N a byte-by-byte gather.
+ * host), and so do 16-byte aligned streams with F*N % 16 == 0 and F*N <= 65536 (as one channel of F*N columns);
+ * other shapes a byte-by-byte gather.
  * Enqueues on `stream`, does not synchronise.  Returns CORR_OK or an error code. */
 int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int32_t *lags_dev,
                     uint8_t *packed_out_dev, corr_stream_t stream);

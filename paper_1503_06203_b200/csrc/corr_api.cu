@@ -594,7 +594,11 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
         return CORR_ERR_INVALID_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    if (N % 16 != 0 || (N + 127) / 128 > corr::SH_MAX_GROUPS) {
+    // N % 16 != 0 but rows of a multiple of 16 bytes: one channel of F * N columns whose lags repeat with period N
+    const bool flat = N % 16 != 0 && ((long long)F * N) % 16 == 0 && (long long)F * N <= 128 * corr::SH_MAX_GROUPS &&
+                      !((reinterpret_cast<uintptr_t>(packed_in_dev) | reinterpret_cast<uintptr_t>(packed_out_dev)) & 15u);
+    const int Nk = flat ? F * N : N, Fk = flat ? 1 : F;
+    if (Nk % 16 != 0 || (Nk + 127) / 128 > corr::SH_MAX_GROUPS) {
         dim3 grid((unsigned)((N + 127) / 128), (unsigned)F, (unsigned)((T + corr::SH_TB - 1) / corr::SH_TB));
         corr::corr_shift_bytes_kernel<<<grid, 256, 0, stream>>>(packed_in_dev, packed_out_dev, lags_dev, N, F, T);
         CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
@@ -606,8 +610,8 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
     }
     // the input as a 3-D byte tensor, innermost first: (N, F, T); a box is 16 rows of 128 inputs of one channel
     CUtensorMap tmap;
-    const cuuint64_t dims[3] = {(cuuint64_t)N, (cuuint64_t)F, (cuuint64_t)T};
-    const cuuint64_t strides[2] = {(cuuint64_t)N, (cuuint64_t)F * (cuuint64_t)N};
+    const cuuint64_t dims[3] = {(cuuint64_t)Nk, (cuuint64_t)Fk, (cuuint64_t)T};
+    const cuuint64_t strides[2] = {(cuuint64_t)Nk, (cuuint64_t)Fk * (cuuint64_t)Nk};
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)corr::SH_BOX_ROWS};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     CUresult r = get_encode_fn()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_in_dev), dims, strides,
@@ -623,10 +627,10 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
     // the attribute belongs to the current device's context: set it on every call (a host-side table write)
     CUDA_TRY(cudaFuncSetAttribute(corr::corr_shift_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::SH_SMEM_BYTES),
              CORR_ERR_CUDA);
-    const long long tiles = (long long)((N + 127) / 128) * F * ((T + corr::SH_TB - 1) / corr::SH_TB);
+    const long long tiles = (long long)((Nk + 127) / 128) * Fk * ((T + corr::SH_TB - 1) / corr::SH_TB);
     const unsigned grid = (unsigned)std::min<long long>(tiles, sms);
     corr::corr_shift_kernel<<<grid, corr::SH_THREADS, corr::SH_SMEM_BYTES, stream>>>(tmap, packed_in_dev, packed_out_dev, lags_dev,
-                                                                                   N, F, T);
+                                                                                   Nk, Fk, T, N);
     CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
     return CORR_OK;
 }

@@ -60,9 +60,11 @@ corr_shift_bytes_kernel(const uint8_t *__restrict__ in, uint8_t *__restrict__ ou
 }
 
 // N % 16 == 0.  tmap: the input as the 3-D byte tensor (N, F, T), box (128, 1, SH_BOX_ROWS), no swizzle.
+// Column n of a row has the lag lags[n % nlag]: nlag = N, or -- a stream whose N is not a multiple of 16 but whose rows
+// are (F * N_stream % 16 == 0), seen as ONE channel of N = F * N_stream columns -- nlag = N_stream.
 __global__ void __launch_bounds__(SH_THREADS, 1)
 corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__restrict__ in, uint8_t *__restrict__ out,
-                  const int *__restrict__ lags, int N, int F, int T)
+                  const int *__restrict__ lags, int N, int F, int T, int nlag)
 {
     extern __shared__ uint8_t sh_raw[];
     const uint32_t base = (ptx::smem_u32(sh_raw) + 127u) & ~127u;
@@ -90,7 +92,7 @@ corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__res
 #pragma unroll
         for (int j = 0; j < 4; ++j)
             if (g * 128 + 4 * lane + j < N) {
-                const int l = __ldg(lags + g * 128 + 4 * lane + j);
+                const int l = __ldg(lags + (g * 128 + 4 * lane + j) % nlag);
                 lo = min(lo, l);
                 hi = max(hi, l);
             }
@@ -183,7 +185,15 @@ corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__res
             const int ncols = min(128, N - n0);
             const int slot = k % SH_SLOTS;
             int4 lv = make_int4(0, 0, 0, 0);   // the lags of this thread's four inputs
-            if (4 * lane < ncols) lv = __ldg(reinterpret_cast<const int4 *>(lags + n0) + lane);
+            if (4 * lane < ncols) {
+                if (nlag == N) {
+                    lv = __ldg(reinterpret_cast<const int4 *>(lags + n0) + lane);
+                } else {
+                    const int c = n0 + 4 * lane;
+                    lv = make_int4(__ldg(lags + c % nlag), __ldg(lags + (c + 1) % nlag), __ldg(lags + (c + 2) % nlag),
+                                   __ldg(lags + (c + 3) % nlag));
+                }
+            }
             ptx::mbar_wait(full(slot), (uint32_t)((k / SH_SLOTS) & 1));
             const int4 m = meta[slot];
             uint8_t *win = ring + m.x * 128;
@@ -234,12 +244,12 @@ corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__res
                 const int tcw = min(4 * SH_TB, T - t0);
                 const int c16n = ncols >> 4;
                 const int w = ct & 3, rl = ct >> 2;
-                const int *lg = lags + n0;
+                auto lag_of = [&](int n) { return __ldg(lags + (n0 + n) % nlag); };
                 for (int c = 0; c < c16n; ++c) {
                     int glo = 0x7fffffff, ghi = (int)0x80000000;
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
-                        const int l = __ldg(lg + 16 * c + j);
+                        const int l = lag_of(16 * c + j);
                         glo = min(glo, l);
                         ghi = max(ghi, l);
                     }
@@ -254,8 +264,8 @@ corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__res
                             *reinterpret_cast<uint4 *>(win + r * 16) = v;
                         }
                         ptx::named_bar_sync(1, SH_CTHREADS);
-                        const int o0 = (ghi - __ldg(lg + 16 * c + 4 * w + 0)) * 16 + 4 * w + 0, o1 = (ghi - __ldg(lg + 16 * c + 4 * w + 1)) * 16 + 4 * w + 1;
-                        const int o2 = (ghi - __ldg(lg + 16 * c + 4 * w + 2)) * 16 + 4 * w + 2, o3 = (ghi - __ldg(lg + 16 * c + 4 * w + 3)) * 16 + 4 * w + 3;
+                        const int o0 = (ghi - lag_of(16 * c + 4 * w + 0)) * 16 + 4 * w + 0, o1 = (ghi - lag_of(16 * c + 4 * w + 1)) * 16 + 4 * w + 1;
+                        const int o2 = (ghi - lag_of(16 * c + 4 * w + 2)) * 16 + 4 * w + 2, o3 = (ghi - lag_of(16 * c + 4 * w + 3)) * 16 + 4 * w + 3;
                         for (int tr = rl; tr < tcw; tr += SH_CTHREADS / 4) {
                             const uint8_t *rowp = win + tr * 16;
                             const uint32_t b0 = rowp[o0], b1 = rowp[o1], b2 = rowp[o2], b3 = rowp[o3];
@@ -265,7 +275,7 @@ corr_shift_kernel(const __grid_constant__ CUtensorMap tmap, const uint8_t *__res
                     } else {
                         for (int idx = ct; idx < tcw * 16; idx += SH_CTHREADS) {
                             const int tr = idx >> 4, n = 16 * c + (idx & 15);
-                            const long long tin = (long long)t0 + tr - __ldg(lg + n);
+                            const long long tin = (long long)t0 + tr - lag_of(n);
                             uint8_t b = 0x88;
                             if (tin >= 0 && tin < T) b = in[((size_t)tin * F + f) * (size_t)N + n0 + n];
                             out[((size_t)(t0 + tr) * F + f) * (size_t)N + n0 + n] = b;

@@ -74,7 +74,8 @@ def _gpu_shift(corr, packed, lags):
 @pytest.mark.gpu
 def test_time_shift_parity(corr, oracle):
     rng = np.random.default_rng(17)
-    shapes = [(1, 1, 1), (300, 2, 16), (257, 3, 48), (1000, 2, 272), (513, 1, 2048), (700, 2, 100), (50, 3, 5)]
+    shapes = [(1, 1, 1), (300, 2, 16), (257, 3, 48), (1000, 2, 272), (513, 1, 2048), (700, 2, 100), (50, 3, 5),
+              (900, 4, 100), (400, 16, 37)]      # the last two: N % 16 != 0 with rows of a multiple of 16 bytes
     for (T, F, N) in shapes:
         packed = rng.integers(0, 256, (T, F, N), dtype=np.uint8)
         for spread in (0, 3, 200, 1500, 5000):              # 1500+: wider than the staged window -> general path
