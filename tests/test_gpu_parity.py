@@ -482,6 +482,39 @@ def _config_case(corr, oracle, name, path=0):
     assert np.array_equal(got, want), f"{name}: {(got != want).sum()} mismatches"
 
 
+@pytest.mark.parametrize("shape", [(20000, 1, 300), (40000, 2, 64)])
+def test_very_large_n_sampled(corr, oracle, shape):
+    # sizes the oracle cannot finish whole (0.8 and 3.2 G complex MACs per sample, up to 1.6 G baselines): sampled
+    # baselines one by one (oracle.pair) at the corners, around the edges of the 128-blocks and at random; every
+    # baseline written (none left at the fill value, which no sum can reach); the diagonal against the power sums
+    import torch
+    N, F, T = shape
+    rng = np.random.default_rng(N)
+    packed = rng.integers(0, 256, (T, F, N), dtype=np.uint8)
+    fill = -2 ** 31
+    with corr.Plan(N, F, T) as plan:
+        vis = plan.new_vis()
+        vis.fill_(fill)
+        plan.execute(torch.from_numpy(packed).cuda(), vis)
+        torch.cuda.synchronize()
+        assert int((vis == fill).sum().item()) == 0
+        xs, ys = list(rng.integers(0, N, 300)), list(rng.integers(0, N, 300))
+        for e in (0, 1, 127, 128, 129, N - 129, N - 128, N - 2, N - 1):
+            for g in (0, 127, 128, N - 1):
+                xs.append(e)
+                ys.append(g)
+        for f in range(F):
+            idx = [oracle.baseline_index(N, int(min(x, y)), int(max(x, y))) for x, y in zip(xs, ys)]
+            got = vis[f, torch.tensor(idx, device="cuda")].cpu().numpy()
+            for (x, y), g in zip(zip(xs, ys), got):
+                assert tuple(g) == tuple(oracle.pair(packed, f, int(min(x, y)), int(max(x, y)))), (f, x, y)
+        re, im = (packed >> 4).astype(np.int64) - 8, (packed & 15).astype(np.int64) - 8
+        power = (re * re + im * im).sum(axis=0)                                  # [F][N]
+        diag = torch.tensor([oracle.baseline_index(N, x, x) for x in range(N)], device="cuda")
+        got = vis[:, diag].cpu().numpy()
+        assert np.array_equal(got[..., 0], power) and not got[..., 1].any()
+
+
 def test_cfg1(corr, oracle):
     _config_case(corr, oracle, "cfg1")
 
