@@ -76,7 +76,8 @@ enum {
  * (TMA strides and box start addresses are multiples of 16 bytes); CORR_PATH_DP4A takes any N without a copy and is
  * only used on request.  Testing aids (environment, read at plan creation): CORR_FORCE_PATH=dp4a|tcgen05|imma
  * overrides the choice; CORR_TC_VARIANT=1|3|5 forces the tcgen05 kernel (1 single-CTA tiles, 3 CTA pairs, 5 = CTA
- * pairs with three products per complex MAC on the stored bytes and the Eq. 3 offset correction). */
+ * pairs with three products per complex MAC on the stored bytes and the Eq. 3 offset correction).
+ * CORR_NO_PDL (read at every corr_execute) launches the CTA-pair kernel without programmatic stream serialisation. */
 corr_plan *corr_plan_create(int N, int F, int T);
 
 /* Same, with the path given explicitly (CORR_PATH_*).  CORR_ERR_UNSUPPORTED -> NULL if the

@@ -766,7 +766,22 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             if (p->variant == 5)
                 corr::corr_tc5_kernel<<<p->grid, corr::T5_THREADS, corr::T5_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
             else
-                corr::corr_tc3_kernel<<<p->grid, corr::T3_THREADS, corr::T3_SMEM_BYTES, stream>>>(p->tmap, p->tmap_y, prm);
+            {
+                // programmatic dependent launch: the CTAs of this launch may take the SMs the previous kernel of the
+                // stream frees one by one and run their prologue (barriers, TMEM, cluster handshake) there; they touch
+                // global memory only after griddepcontrol.wait, i.e. after that kernel has completed
+                cudaLaunchConfig_t cfg = {};
+                cfg.gridDim = dim3((unsigned)p->grid);
+                cfg.blockDim = dim3(corr::T3_THREADS);
+                cfg.dynamicSmemBytes = corr::T3_SMEM_BYTES;
+                cfg.stream = stream;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                at[0].val.programmaticStreamSerializationAllowed = getenv("CORR_NO_PDL") ? 0 : 1;
+                cfg.attrs = at;
+                cfg.numAttrs = 1;
+                CUDA_TRY(cudaLaunchKernelEx(&cfg, corr::corr_tc3_kernel, p->tmap, p->tmap_y, prm), CORR_ERR_CUDA);
+            }
         } else {
             corr::TcParams prm;
             prm.N = (p->pack_sub == 64) ? 128 : p->N;

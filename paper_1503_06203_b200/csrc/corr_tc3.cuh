@@ -245,6 +245,7 @@ corr_tc3_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     ptx::tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot_g;
     if (tmem != 0) __trap();  // all 512 columns were requested: the allocation starts at lane 0, column 0
+    ptx::grid_dependency_wait();   // the previous kernel of the stream has completed: its output (our input, vis, the flags) is visible
 
     Tc3Iter sit = tc3_iter(p, pair, npairs);   // every role walks the same list of segments
     Tc3Seg sg;
