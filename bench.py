@@ -85,6 +85,7 @@ class ClockSampler:
 
     def __init__(self, index: int):
         self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.t_begin = None    # samples before begin() (taken while the device warms up) are not reported
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -107,19 +108,29 @@ class ClockSampler:
         }
         while not self._stop.is_set():
             try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
                 mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for k, bit in names.items():
-                    if mask & bit:
-                        self.reasons.add(k)
+                if self.t_begin is not None:
+                    self.samples.append(mhz)
+                    for k, bit in names.items():
+                        if mask & bit:
+                            self.reasons.add(k)
             except Exception:
                 pass
             time.sleep(0.002)
 
-    def start(self):
+    def start(self, recording: bool = True):
+        """recording=False: the thread polls but keeps nothing until begin() (NVML start-up and the thread start stay
+        out of the gap between the warm-up and the timed region: after some ten milliseconds of idling the part needs
+        about fifteen 0.3 ms steps to get back to its full speed)."""
+        if recording:
+            self.t_begin = time.perf_counter()
         if self.nv is not None:
             self._thread = threading.Thread(target=self._loop, daemon=True)
             self._thread.start()
+
+    def begin(self):
+        self.t_begin = time.perf_counter()
 
     def stop(self):
         if self._thread is not None:
@@ -277,14 +288,14 @@ def main():
 
     # the int8 ceiling of THIS device: a bare issue loop of the hot path's own tcgen05.mma.kind::i8 (~3 ms each).  Measured
     # before the timed region (it also brings the part out of its idle clocks, which W = 5 steps of 0.3 ms do not)
+    sampler = ClockSampler(local_rank)
+    sampler.start(recording=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     int8_measured = max(corr.corr_measure_int8_tops(20000), corr.corr_measure_int8_tops(20000))
     for i in range(args.warmup):
         plan.execute(dev_inputs[i % NBUF], vis)
     barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    sampler.begin()
     e0.record(stream)
     for i in range(args.steps):
         plan.execute(dev_inputs[i % NBUF], vis)
