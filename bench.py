@@ -174,7 +174,14 @@ def config_table(corr, dev, peaks, reps=20):
         nbuf = 2 if N * F * T >= (64 << 20) else 8
         ins = [torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device=dev) for _ in range(nbuf)]
         vis = torch.zeros((F, plan.baselines, 2), dtype=torch.int32, device=dev)
+        # warm-up: 3 calls, then as many as make 8 ms of work (after the allocations above the part has idled, and it
+        # takes some 5 ms of load to get back to full speed)
+        e0.record()
         for i in range(3):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        e1.record()
+        torch.cuda.synchronize(dev)
+        for i in range(min(400, int(8.0 / max(e0.elapsed_time(e1) / 3, 1e-3)))):
             plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
         torch.cuda.synchronize(dev)
         e0.record()

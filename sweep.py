@@ -43,7 +43,12 @@ def other_op(args):
                 "shared by 16 inputs +-16": torch.randint(-16, 17, ((n + 15) // 16,), dtype=torch.int32, device=dev).repeat_interleave(16)[:n].contiguous(),
                 "independent +-256": torch.randint(-256, 257, (n,), dtype=torch.int32, device=dev)}
         for name, lags in pats.items():
+            e0.record()
             for _ in range(3):
+                time_shift(a, lags, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            for _ in range(min(400, int(8.0 / max(e0.elapsed_time(e1) / 3, 1e-3)))):   # 8 ms of warm-up, see main()
                 time_shift(a, lags, out=out)
             torch.cuda.synchronize()
             e0.record()
@@ -59,7 +64,7 @@ def other_op(args):
         gate = ((np.arange(t) % 64) * 4 // 64).astype(np.int32)
         vis = plan.execute_gated(a, gate, 4)
         run = lambda: plan.execute_gated(a, gate, 4, vis=vis)
-    for _ in range(3):
+    for _ in range(20):    # 8 ms of warm-up, see main()
         run()
     torch.cuda.synchronize()
     e0.record()
@@ -96,10 +101,17 @@ def main():
         nbuf = 2 if N * F * T >= (64 << 20) else 8
         ins = [torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device=dev) for _ in range(nbuf)]
         vis = torch.zeros((F, plan.baselines, 2), dtype=torch.int32, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        # warm-up: 3 calls, then as many as make 8 ms of work (after the allocations above the part has idled, and it
+        # takes some 5 ms of load to get back to full speed: profiles/r02_tc3_ncu_summary.md)
+        e0.record()
         for i in range(3):
             plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        e1.record()
         torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(min(400, int(8.0 / max(e0.elapsed_time(e1) / 3, 1e-3)))):
+            plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
+        torch.cuda.synchronize()
         e0.record()
         for i in range(args.reps):
             plan.execute(ins[i % nbuf], vis, accumulate=bool(acc))
