@@ -205,6 +205,29 @@ int corr_count_tiles(int N, int tile_x, int tile_y);
  * Returns CORR_OK or CORR_ERR_INVALID_ARG. */
 int corr_schedule_pairs(int N, int F, int T, int pairs, int info[8], int *pieces);
 
+/* corr_execute_noalloc -- one correlation pass (Eq. 1, summed over time PAPER.md:48, upper triangle
+ * PAPER.md:50; the same result as corr_execute on a plan for (N, F, T)) for small N WITHOUT a plan and without any
+ * allocation: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it).  The scratch memory a plan would own for this path -- the copy of the stream padded to the next
+ * multiple of 16 inputs, needed when N % 16 != 0 -- is a static device array of CORR_NOALLOC_MAX_BYTES inside the
+ * library, which every GPU that loads the library holds until the process exits.
+ *   N           1 <= N <= 64 (the warp-MMA kernel of CORR_PATH_IMMA; larger N: CORR_ERR_UNSUPPORTED, use a plan)
+ *   F, T        as for corr_plan_create; when N % 16 != 0 the padded stream T * F * ceil16(N) bytes must fit
+ *               CORR_NOALLOC_MAX_BYTES, else CORR_ERR_UNSUPPORTED with the sizes in corr_last_error()
+ *   packed_dev  DEVICE pointer, T*F*N bytes, layout [T][F][N]; 16-byte aligned when N % 16 == 0; read only
+ *   vis_dev     DEVICE pointer, F*N(N+1)/2*2 int32, layout [F][B][2]; 8-byte aligned; caller-owned
+ *   accumulate_flag  as for corr_execute
+ * Enqueues on `stream` (the pad copy when needed, a memset of vis_dev when T is split and the call overwrites, the
+ * kernel) and returns without synchronising; calls no cudaMalloc / cudaFree or allocating library routine (the first
+ * call on a device looks up the array's address and sets kernel attributes).  ALL calls on a device share the one
+ * scratch array, which keeps the previous call's contents (every byte a call reads it has written itself first):
+ * calls that overlap on the GPU -- two streams, or two host threads on two streams -- race on it; keep them on one
+ * stream or order them with events.  Returns CORR_OK or an error code. */
+#define CORR_NOALLOC_MAX_BYTES (32u << 20)   /* 32 MiB of device memory per GPU, held from library load to exit */
+#define CORR_NOALLOC_MAX_DEVICES 64
+int corr_execute_noalloc(int N, int F, int T, const uint8_t *packed_dev, int32_t *vis_dev, int accumulate_flag,
+                         corr_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -7,8 +7,8 @@ sm_100 device, calls raise.
 """
 from .binding import (CorrError, Plan, PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA, baseline_index, count_tiles, schedule_pairs,
                       corr_execute, corr_execute_gated, corr_submit_host, corr_wait_host, corr_measure_int8_tops, corr_plan_create, corr_plan_destroy, corr_time_shift, lib_path, load_library,
-                      time_shift)
+                      time_shift, corr_execute_noalloc, execute_noalloc, NOALLOC_MAX_BYTES)
 
 __all__ = ["CorrError", "Plan", "PATH_AUTO", "PATH_DP4A", "PATH_TCGEN05", "PATH_IMMA", "baseline_index", "count_tiles", "schedule_pairs",
            "corr_execute", "corr_execute_gated", "corr_submit_host", "corr_wait_host", "corr_measure_int8_tops", "corr_plan_create", "corr_plan_destroy", "corr_time_shift", "lib_path", "load_library",
-           "time_shift"]
+           "time_shift", "corr_execute_noalloc", "execute_noalloc", "NOALLOC_MAX_BYTES"]

@@ -12,7 +12,7 @@ PATH_AUTO, PATH_DP4A, PATH_TCGEN05, PATH_IMMA = 0, 1, 2, 3
 # every symbol include/corr.h declares (tests check the library exports all of them)
 SYMBOLS = ("corr_plan_create", "corr_plan_create_ex", "corr_execute", "corr_execute_host",
            "corr_plan_destroy", "corr_last_error", "corr_input_bytes", "corr_vis_elems",
-           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_schedule_pairs", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops", "corr_submit_host", "corr_wait_host")
+           "corr_baseline_index", "corr_plan_info", "corr_count_tiles", "corr_schedule_pairs", "corr_time_shift", "corr_execute_gated", "corr_measure_int8_tops", "corr_submit_host", "corr_wait_host", "corr_execute_noalloc")
 
 
 class CorrError(RuntimeError):
@@ -69,6 +69,8 @@ def load_library():
         lib.corr_measure_int8_tops.restype = ci
         lib.corr_time_shift.argtypes = [ci, ci, ci, vp, vp, vp, vp]
         lib.corr_time_shift.restype = ci
+        lib.corr_execute_noalloc.argtypes = [ci, ci, ci, vp, vp, ci, vp]
+        lib.corr_execute_noalloc.restype = ci
         _lib = lib
     return _lib
 
@@ -135,6 +137,30 @@ def time_shift(packed, lags, out=None, stream=None):
     s = torch.cuda.current_stream(packed.device) if stream is None else stream
     corr_time_shift(N, F, T, packed.data_ptr(), lags.data_ptr(), out.data_ptr(), s.cuda_stream)
     return out
+
+
+NOALLOC_MAX_BYTES = 32 << 20   # CORR_NOALLOC_MAX_BYTES of include/corr.h
+
+
+def corr_execute_noalloc(N: int, F: int, T: int, packed_dev_ptr: int, vis_dev_ptr: int, accumulate_flag: int, stream: int) -> None:
+    rc = load_library().corr_execute_noalloc(N, F, T, packed_dev_ptr, vis_dev_ptr, int(bool(accumulate_flag)), stream)
+    if rc != 0:
+        raise CorrError(f"corr_execute_noalloc -> {rc}: {_err()}")
+
+
+def execute_noalloc(packed, vis, accumulate=False, stream=None):
+    """packed: uint8 CUDA tensor [T][F][N], N <= 64; vis: int32 CUDA tensor [F][N(N+1)/2][2] (the caller allocates it:
+    this call allocates nothing, see corr_execute_noalloc in include/corr.h).  Enqueues only; returns vis."""
+    import torch
+    if not packed.is_cuda or packed.dtype != torch.uint8 or not packed.is_contiguous() or packed.dim() != 3:
+        raise ValueError("packed must be a contiguous uint8 CUDA tensor [T][F][N]")
+    T, F, N = packed.shape
+    if (not vis.is_cuda or vis.dtype != torch.int32 or not vis.is_contiguous()
+            or tuple(vis.shape) != (F, N * (N + 1) // 2, 2)):
+        raise ValueError("vis must be a contiguous int32 CUDA tensor [F][N(N+1)/2][2]")
+    s = torch.cuda.current_stream(packed.device) if stream is None else stream
+    corr_execute_noalloc(N, F, T, packed.data_ptr(), vis.data_ptr(), accumulate, s.cuda_stream)
+    return vis
 
 
 def corr_submit_host(plan: int, packed_host_ptr: int, vis_host_ptr: int, accumulate_flag: int, stream: int) -> None:

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <mutex>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -1075,6 +1076,179 @@ int corr_execute_host(corr_plan *p, const uint8_t *packed_host, int32_t *vis_hos
     int rc = corr_submit_host(p, packed_host, vis_host, accumulate_flag, stream_);
     if (rc != CORR_OK) return rc;
     return corr_wait_host(p);
+}
+
+
+}  // extern "C"
+
+// ---------------------------------------------------------------- corr_execute_noalloc
+// For callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the small-N pass without a plan.  What a plan owns for this path is one piece of scratch memory, the
+// copy of the stream padded to a multiple of 16 inputs (corr_pad_kernel writes it, corr_imma_kernel reads it through
+// TMA); here that scratch is a file-scope array every GPU that loads the library holds until exit.  In host code the
+// array's name is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress, once per
+// device, with that device current.
+static __device__ __align__(256) uint8_t g_noalloc_scratch[CORR_NOALLOC_MAX_BYTES];
+
+namespace {
+struct NoallocDevice {
+    bool ready;
+    uint8_t *scratch;   // device address of g_noalloc_scratch on this device
+    int sms;
+    int occ[4];         // resident CTAs per SM of corr_imma_kernel<1..4>
+};
+NoallocDevice g_noalloc_dev[CORR_NOALLOC_MAX_DEVICES];
+std::mutex g_noalloc_mutex;
+
+template <int NT16> cudaError_t noalloc_setup_kernel(int *occ)
+{
+    cudaError_t e = cudaFuncSetAttribute(corr::corr_imma_kernel<NT16>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::IM_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, corr::corr_imma_kernel<NT16>, corr::ImmaCfg<NT16>::THREADS, corr::IM_SMEM_BYTES);
+    return e;
+}
+
+// Set-up of the current device (first call on it): the scratch array's device address and the launch attributes.
+int noalloc_device(const NoallocDevice **out)
+{
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev), CORR_ERR_CUDA);
+    if (dev < 0 || dev >= CORR_NOALLOC_MAX_DEVICES) {
+        set_err("corr_execute_noalloc: device ordinal %d is beyond the %d this entry point keeps state for", dev, CORR_NOALLOC_MAX_DEVICES);
+        return CORR_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoallocDevice &d = g_noalloc_dev[dev];
+    if (!d.ready) {
+        void *ptr = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&ptr, g_noalloc_scratch), CORR_ERR_CUDA);
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) {
+            set_err("corr_execute_noalloc: cudaGetSymbolAddress gave %p for the scratch array", ptr);
+            return CORR_ERR_CUDA;
+        }
+        CUDA_TRY(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev), CORR_ERR_CUDA);
+        CUDA_TRY(noalloc_setup_kernel<1>(&d.occ[0]), CORR_ERR_CUDA);
+        CUDA_TRY(noalloc_setup_kernel<2>(&d.occ[1]), CORR_ERR_CUDA);
+        CUDA_TRY(noalloc_setup_kernel<3>(&d.occ[2]), CORR_ERR_CUDA);
+        CUDA_TRY(noalloc_setup_kernel<4>(&d.occ[3]), CORR_ERR_CUDA);
+        for (int i = 0; i < 4; ++i)
+            if (d.occ[i] < 1) {
+                set_err("corr_execute_noalloc: cannot reserve %d B of shared memory per CTA", corr::IM_SMEM_BYTES);
+                return CORR_ERR_CUDA;
+            }
+        d.scratch = static_cast<uint8_t *>(ptr);
+        d.ready = true;
+    }
+    *out = &d;
+    return CORR_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int corr_execute_noalloc(int N, int F, int T, const uint8_t *packed_dev, int32_t *vis_dev, int accumulate_flag,
+                         corr_stream_t stream_)
+{
+    if (N < 1 || N > 64 || F < 1 || T < 1 || T > 16777215) {
+        set_err("corr_execute_noalloc: need 1 <= N <= 64, F >= 1, 1 <= T <= 16777215 (got N=%d F=%d T=%d)", N, F, T);
+        return (N > 64) ? CORR_ERR_UNSUPPORTED : CORR_ERR_INVALID_ARG;
+    }
+    if (!packed_dev || !vis_dev || (reinterpret_cast<uintptr_t>(vis_dev) & 7u)) {
+        set_err("corr_execute_noalloc: NULL buffer, or vis_dev not 8-byte aligned");
+        return CORR_ERR_INVALID_ARG;
+    }
+    const int n_pad = (N + 15) / 16 * 16;
+    const bool padded = n_pad != N;
+    const unsigned long long need = padded ? (unsigned long long)T * (unsigned long long)F * (unsigned long long)n_pad : 0ull;
+    if (need > (unsigned long long)CORR_NOALLOC_MAX_BYTES) {
+        set_err("corr_execute_noalloc: the padded stream T*F*%d = %llu bytes exceeds the static scratch of %llu bytes "
+                "(CORR_NOALLOC_MAX_BYTES); use a plan (corr_plan_create + corr_execute) for this size",
+                n_pad, need, (unsigned long long)CORR_NOALLOC_MAX_BYTES);
+        return CORR_ERR_UNSUPPORTED;
+    }
+    if ((unsigned long long)F * (unsigned long long)n_pad > 0x7fffffffull) {
+        set_err("corr_execute_noalloc: F*N too large");
+        return CORR_ERR_INVALID_ARG;
+    }
+    if (!padded && (reinterpret_cast<uintptr_t>(packed_dev) & 15u)) {
+        set_err("corr_execute_noalloc: packed_dev must be 16-byte aligned when N is a multiple of 16");
+        return CORR_ERR_INVALID_ARG;
+    }
+    if (!get_encode_fn()) {
+        set_err("corr_execute_noalloc: cuTensorMapEncodeTiled not available from the driver");
+        return CORR_ERR_CUDA;
+    }
+    const NoallocDevice *d = nullptr;
+    int rc = noalloc_device(&d);
+    if (rc != CORR_OK) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+
+    // ---- the schedule corr_plan_create makes for this path: strips of 128 / n_pad channels x chunks of time samples
+    const int nt16 = n_pad / 16, fb = 128 / n_pad;
+    const int strips = (F + fb - 1) / fb;
+    const int slots = d->sms * d->occ[nt16 - 1];
+    const int min_chunks = (T + corr::IM_MAX_CHUNK - 1) / corr::IM_MAX_CHUNK;   // int32 headroom of a chunk
+    int chunks = min_chunks;
+    double best = 0.0;
+    for (int c = min_chunks; c <= std::max(min_chunks, std::min(T / 512, 4 * slots / strips + 1)); ++c) {
+        const long long units = (long long)strips * c;
+        const double eff = (double)units / (double)(((units + slots - 1) / slots) * slots);
+        if (eff > best + 0.10) { best = eff; chunks = c; }
+    }
+    const int t_per_chunk = ((T + chunks - 1) / chunks + corr::IM_ROWS - 1) / corr::IM_ROWS * corr::IM_ROWS;
+    const int slices = (T + t_per_chunk - 1) / t_per_chunk;
+    if (strips > 0x7fffffff / std::max(1, slices) || slices > 65535) {
+        set_err("corr_execute_noalloc: too many work units");
+        return CORR_ERR_INVALID_ARG;
+    }
+
+    // ---- N % 16 != 0: pad into the static scratch.  Every byte the pass reads is written here first, so nothing has
+    //      to be cleared although the array keeps the last call's contents
+    const uint8_t *src = packed_dev;
+    if (padded) {
+        corr::corr_pad_kernel<<<8 * d->sms, 256, 0, stream>>>(packed_dev, d->scratch, N, n_pad, (long long)T * F);
+        CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+        src = d->scratch;
+    }
+    int out_mode;
+    if (slices > 1) {
+        out_mode = corr::OUT_ATOMIC;
+        if (!accumulate_flag)
+            CUDA_TRY(cudaMemsetAsync(vis_dev, 0, (size_t)F * ((size_t)N * (N + 1) / 2) * 2 * sizeof(int32_t), stream), CORR_ERR_CUDA);
+    } else {
+        out_mode = accumulate_flag ? corr::OUT_RMW : corr::OUT_STORE;
+    }
+    // the stream as a byte matrix, innermost first: (F * n_pad, T)
+    CUtensorMap tmap;
+    const cuuint64_t dims2[2] = {(cuuint64_t)F * (cuuint64_t)n_pad, (cuuint64_t)T};
+    const cuuint64_t strides2[1] = {(cuuint64_t)F * (cuuint64_t)n_pad};
+    const cuuint32_t box2[2] = {128u, (cuuint32_t)corr::IM_ROWS};
+    const cuuint32_t estr2[2] = {1u, 1u};
+    CUresult r2 = get_encode_fn()(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(src), dims2, strides2, box2, estr2,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r2 != CUDA_SUCCESS) {
+        set_err("corr_execute_noalloc: cuTensorMapEncodeTiled failed with CUresult %d (N=%d F=%d T=%d)", (int)r2, N, F, T);
+        return CORR_ERR_CUDA;
+    }
+    corr::ImmaParams prm;
+    prm.N = N;
+    prm.F = F;
+    prm.T = T;
+    prm.t_per_chunk = t_per_chunk;
+    prm.out_mode = out_mode;
+    prm.vis = vis_dev;
+    dim3 grid((unsigned)strips, (unsigned)slices);
+    if (nt16 == 1)
+        corr::corr_imma_kernel<1><<<grid, corr::ImmaCfg<1>::THREADS, corr::IM_SMEM_BYTES, stream>>>(tmap, prm);
+    else if (nt16 == 2)
+        corr::corr_imma_kernel<2><<<grid, corr::ImmaCfg<2>::THREADS, corr::IM_SMEM_BYTES, stream>>>(tmap, prm);
+    else if (nt16 == 3)
+        corr::corr_imma_kernel<3><<<grid, corr::ImmaCfg<3>::THREADS, corr::IM_SMEM_BYTES, stream>>>(tmap, prm);
+    else
+        corr::corr_imma_kernel<4><<<grid, corr::ImmaCfg<4>::THREADS, corr::IM_SMEM_BYTES, stream>>>(tmap, prm);
+    CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);
+    return CORR_OK;
 }
 
 }  // extern "C"
