@@ -71,11 +71,12 @@ enum {
  *   T  time samples per corr_execute call, 1 <= T <= 16 777 215
  * Returns NULL on failure; the reason is in corr_last_error().
  * Automatic choice: N <= 64 -> CORR_PATH_IMMA (except N = 64 with an even F: two channels per tcgen05 tile), larger
- * N -> CORR_PATH_TCGEN05 (single-CTA 128 x 128 tiles up to N = 128, CTA-pair 256 x 128 tiles above).  When
+ * N -> CORR_PATH_TCGEN05 (one CTA per channel's 128 x 128 block up to N = 128, CTA-pair 256 x 128 tiles above).  When
  * N % 16 != 0 these two paths first copy the stream to a plan-owned buffer padded to the next multiple of 16 inputs
  * (TMA strides and box start addresses are multiples of 16 bytes); CORR_PATH_DP4A takes any N without a copy and is
  * only used on request.  Testing aids (environment, read at plan creation): CORR_FORCE_PATH=dp4a|tcgen05|imma
- * overrides the choice; CORR_TC_VARIANT=1|3|5 forces the tcgen05 kernel (1 single-CTA tiles, 3 CTA pairs, 5 = CTA
+ * overrides the choice; CORR_TC_VARIANT=1|3|5 forces the tcgen05 kernel (1 single-CTA tiles with both operands in
+ * shared memory -- the round-1 kernel the N <= 128 kernel replaced --, 3 CTA pairs, 5 = CTA
  * pairs with three products per complex MAC on the stored bytes and the Eq. 3 offset correction).
  * CORR_NO_PDL (read at every corr_execute) launches the CTA-pair kernel without programmatic stream serialisation. */
 corr_plan *corr_plan_create(int N, int F, int T);

@@ -21,6 +21,7 @@
 #include "corr_shift.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc3.cuh"
+#include "corr_tcd.cuh"
 #include "corr_tc5.cuh"
 
 namespace {
@@ -168,8 +169,10 @@ struct corr_plan {
     int aligned;
     // tcgen05 only
     int pack_sub;      // variant 1: 128, or 64 when two 64-input channels are packed into one 128-tile (see below)
-    int variant;       // 1: single-CTA tiles 128x128 (corr_tc.cuh; chosen for N <= 128, where a pair tile would be
-                       // half empty); 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default);
+    int variant;       // 1: single-CTA tiles 128x128, both operands' planes in shared memory (corr_tc.cuh; on request);
+                       // 2: one diagonal 128-block per channel on one CTA, A operand in TMEM (corr_tcd.cuh; chosen
+                       // for N <= 128, where a pair tile would be half empty, and for two 64-input channels per tile);
+                       // 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default above N = 128);
                        // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
     int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
     long long total_groups;
@@ -439,6 +442,8 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         const char *v = getenv("CORR_TC_VARIANT");   // testing aid: force a kernel
         p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "3")) ? 3 : (v && !strcmp(v, "5")) ? 5 : (n_pad <= 128) ? 1 : 3;
         if (packed64) p->variant = 1;
+        // one 128-block per channel: the diagonal-block kernel (A operand in TMEM, corr_tcd.cuh) unless variant 1 is forced
+        if (p->variant == 1 && (packed64 || n_pad <= 128) && !(v && !strcmp(v, "1"))) p->variant = 2;
     }
     p->pack_sub = packed64 ? 64 : 128;
     const int Ns = packed64 ? 128 : N, Fs = packed64 ? F / 2 : F;   // the shape the tile schedule sees
@@ -463,6 +468,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     // ---- split-T: choose the number of T-slices per tile from a wave-count cost model
     const int quantum = (path == CORR_PATH_DP4A) ? corr::DP4A_TK
                         : (p->variant >= 3) ? corr::T3_GROUP  // tc3 / tc5 run whole groups of stages
+                        : (p->variant == 2) ? corr::TD_GROUP
                                             : corr::TC_ST;
     const int max_slice = (path == CORR_PATH_DP4A) ? (1 << 22) : (p->variant == 5) ? corr::T5_MAX_SLICE : corr::TC_MAX_SLICE;
     const int ctas_per_wave = (path == CORR_PATH_DP4A) ? 4 * p->sm_count : (p->variant >= 3 ? p->sm_count / 2 : p->sm_count);
@@ -532,6 +538,8 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
                                               corr::T3_SMEM_BYTES);
         cudaError_t e5 = cudaFuncSetAttribute(corr::corr_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::T5_SMEM_BYTES);
+        if (e5 == cudaSuccess)
+            e5 = cudaFuncSetAttribute(corr::corr_tcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::TD_SMEM_BYTES);
         if (e1 != cudaSuccess || e3 != cudaSuccess || e5 != cudaSuccess) {
             g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
                     corr::T3_SMEM_BYTES, corr::T5_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
@@ -797,7 +805,10 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.out_mode = out_mode;
             prm.tiles = p->tiles_dev;
             prm.vis = vis_dev;
-            corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
+            if (p->variant == 2)
+                corr::corr_tcd_kernel<<<p->grid, corr::TD_THREADS, corr::TD_SMEM_BYTES, stream>>>(p->tmap, prm);
+            else
+                corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
         }
     }
     CUDA_TRY(cudaGetLastError(), CORR_ERR_CUDA);

@@ -1,0 +1,357 @@
+// corr_tcd.cuh -- steps S1-S5 for N <= 128: one 128 x 128 tile per channel, the DIAGONAL block, on one CTA, with the
+// A operand in tensor memory.
+//
+// Same mathematics as the other tcgen05 kernels (Eq. 1, summed over time PAPER.md:48, upper triangle
+// PAPER.md:50; x16 int8 operand planes, results shifted right by 8 in the epilogue).  corr_tc.cuh serves these sizes
+// with both operands' planes in shared memory and moves 768 wavefronts through the shared-memory pipe per 64-sample
+// stage against 512 tensor cycles.  Here, as in corr_tc3.cuh:
+//   * the rows' planes never enter shared memory: ldmatrix.m16n16.x2.trans.b8 transposes the packed block, the
+//     planes 16 Re, 16 Im are formed in registers and written to TMEM with tcgen05.st (A operand of the MMAs);
+//   * rows and columns are the same 128 inputs, so ONE packed block per stage is loaded (8 KB) and the columns'
+//     planes Br, Bi are made from it at the same physical offsets (MN-major, 128-B swizzle as TMA wrote it);
+//   * the epilogue stages the rows of the upper triangle in shared memory and sends them as bulk copies / bulk
+//     reduce-adds; rows 64..127 only hold columns 64..127, which is what lets the image fit beside the rings.
+// Per stage: 64 (ldmatrix) + 64 (loads) + 128 (plane stores) + 256 (tensor-core reads) = 512 wavefronts.
+//
+// TMEM columns:   0..127  IR += Ai Br^T     128..255  Re += Ai Bi^T + Ar Br^T     256..383  RI += Ar Bi^T
+//               384..511  A planes, 4 stages x (Ar 16 columns | Ai 16 columns); lane = input
+//   Re = D[128 + j] >> 8,   Im = (D[j] - D[256 + j]) >> 8.
+// Two whole channels of 64 inputs per tile (TcParams::sub = 64, see corr_tc.cuh): only the two diagonal 64-blocks are
+// written, as channels 2f and 2f + 1.
+//
+// Warps (576 threads, one CTA per SM, persistent over units = (channel, T-slice)):
+//   0 TMA producer | 1 TMEM owner + MMA issue | 2-9 unpack | 10-17 epilogue (lane quarter warp % 4, column half)
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "corr_dp4a.cuh"  // OutMode
+#include "corr_ptx.cuh"
+#include "corr_tc.cuh"    // TcParams
+
+namespace corr {
+
+constexpr int TD_ST = 64;               // time samples per stage
+#ifndef TD_PK_N
+#define TD_PK_N 6
+#endif
+#ifndef TD_PL_N
+#define TD_PL_N 4
+#endif
+constexpr int TD_PK_STAGES = TD_PK_N;   // packed-byte ring
+constexpr int TD_PL_STAGES = TD_PL_N;   // operand ring: TMEM A stage + smem B stage
+constexpr int TD_GROUP = TD_ST * TD_PL_STAGES;   // a unit runs whole groups of stages (static ring positions in the MMA loop)
+constexpr int TD_UNPACK_WARPS = 8;
+constexpr int TD_EPI_WARP0 = 2 + TD_UNPACK_WARPS;
+constexpr int TD_EPI_WARPS = 8;
+constexpr int TD_THREADS = 32 * (TD_EPI_WARP0 + TD_EPI_WARPS);
+constexpr int TD_PK_BYTES = TD_ST * 128;          // the packed block of a stage
+constexpr int TD_PLANE = TD_ST * 128;             // one plane of the columns per stage
+constexpr int TD_PL_BYTES = 2 * TD_PLANE;         // Br, Bi
+constexpr int TD_PITCH_LO = 128 * 8 + 16;         // image of a row 0..63: 128 baselines + parity slot
+constexpr int TD_PITCH_HI = 64 * 8 + 16;          // image of a row 64..127: columns 64..127 + parity slot
+constexpr int TD_EPI_BYTES = 64 * (TD_PITCH_LO + TD_PITCH_HI);
+constexpr int TD_SMEM_BYTES = 1024 + TD_PK_STAGES * TD_PK_BYTES + TD_PL_STAGES * TD_PL_BYTES + TD_EPI_BYTES + 256;
+constexpr uint32_t TD_ACOL0 = 384, TD_ACOLS = 32;
+constexpr int TD_MAX_SLICE = 32768;               // |sum| <= 2 * 128 * 128 * slice < 2^31
+
+__global__ void __launch_bounds__(TD_THREADS, 1)
+corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *gbase = smem_raw + (base - ptx::smem_u32(smem_raw));
+    const uint32_t pk0 = base;
+    const uint32_t pl0 = pk0 + TD_PK_STAGES * TD_PK_BYTES;
+    const uint32_t epi0 = pl0 + TD_PL_STAGES * TD_PL_BYTES;
+    const uint32_t bar0 = epi0 + TD_EPI_BYTES;
+    uint8_t *epi_g = gbase + (epi0 - base);
+    auto pk_full = [&](int s) { return bar0 + 8u * s; };
+    auto pk_empty = [&](int s) { return bar0 + 8u * (TD_PK_STAGES + s); };
+    auto pl_full = [&](int s) { return bar0 + 8u * (2 * TD_PK_STAGES + s); };
+    auto pl_empty = [&](int s) { return bar0 + 8u * (2 * TD_PK_STAGES + TD_PL_STAGES + s); };
+    const uint32_t acc_full = bar0 + 8u * (2 * TD_PK_STAGES + 2 * TD_PL_STAGES);
+    const uint32_t acc_empty = acc_full + 8u;
+    const uint32_t tmem_slot = acc_empty + 8u;
+    volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + (tmem_slot - base));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tmap(&tmap);
+        for (int s = 0; s < TD_PK_STAGES; ++s) {
+            ptx::mbar_init(pk_full(s), 1);
+            ptx::mbar_init(pk_empty(s), TD_UNPACK_WARPS / 2);   // the group of unpack warps that owns the position
+        }
+        for (int s = 0; s < TD_PL_STAGES; ++s) {
+            ptx::mbar_init(pl_full(s), TD_UNPACK_WARPS / 2);
+            ptx::mbar_init(pl_empty(s), 1);
+        }
+        ptx::mbar_init(acc_full, 1);
+        ptx::mbar_init(acc_empty, TD_EPI_WARPS);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc<1>(tmem_slot, 512);
+        ptx::tmem_relinquish<1>();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot_g;
+    if (tmem != 0) __trap();  // all 512 columns were requested: the allocation starts at lane 0, column 0
+
+    // unit u = (channel f, T-slice): samples [t_begin, t_end), run as whole groups of TD_GROUP samples (the stages
+    // beyond t_end are loaded -- TMA fills rows beyond T with zeros -- and masked to zero operands by the unpack)
+    auto unit = [&](int u, int &f, int &t_begin, int &t_end, int &ngroups) {
+        f = u / p.slices;
+        const int slice = u - f * p.slices;
+        t_begin = slice * p.t_per_slice;
+        t_end = min(p.T, t_begin + p.t_per_slice);
+        ngroups = (t_end - t_begin + TD_GROUP - 1) / TD_GROUP;
+    };
+
+    if (warp == 0) {
+        // ===================== S1: TMA producer =====================
+        if (lane == 0) {
+            int st = 0;
+            uint32_t ph = 0;
+            for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+                int f, t_begin, t_end, ngroups;
+                unit(u, f, t_begin, t_end, ngroups);
+                for (int t = t_begin; t < t_begin + ngroups * TD_GROUP; t += TD_ST) {
+                    ptx::mbar_wait(pk_empty(st), ph ^ 1u);
+                    ptx::mbar_arrive_expect_tx(pk_full(st), TD_PK_BYTES);
+                    ptx::tma_load_3d(pk0 + st * TD_PK_BYTES, &tmap, pk_full(st), 0, f, t);
+                    if (++st == TD_PK_STAGES) { st = 0; ph ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== S4: MMA issue =====================
+        // the whole warp runs the loop (warp-uniform operands, compile-time ring positions), one elected lane issues
+        constexpr uint32_t idesc = make_idesc_i8(128, 128, true, true, /*A K-major (TMEM)*/ false, /*B MN-major*/ true);
+        uint32_t ph = 0, acc_ph = 0;
+        const bool issuer = ptx::elect_one();
+        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+            int f, t_begin, t_end, ngroups;
+            unit(u, f, t_begin, t_end, ngroups);
+            ptx::mbar_wait(acc_empty, acc_ph ^ 1u);
+            ptx::tc_fence_after_sync();
+            uint32_t acc = 0;
+            for (int g = 0; g < ngroups; ++g) {
+#pragma unroll
+                for (int st = 0; st < TD_PL_STAGES; ++st) {
+                    ptx::mbar_wait(pl_full(st), ph);
+                    ptx::tc_fence_after_sync();
+                    if (issuer) {
+                        const uint32_t pl = pl0 + st * TD_PL_BYTES;
+                        const uint32_t a0 = TD_ACOL0 + (uint32_t)st * TD_ACOLS;
+#pragma unroll
+                        for (int ks = 0; ks < TD_ST / 32; ++ks) {
+                            // one 128-wide MN block, 128-B swizzle, 8-row K groups 1024 B apart; K-step = 32 rows = 4096 B
+                            const uint64_t dBr = make_smem_desc(pl + ks * 4096, TD_PLANE, 1024, 2);
+                            const uint64_t dBi = make_smem_desc(pl + TD_PLANE + ks * 4096, TD_PLANE, 1024, 2);
+                            const uint32_t a_r = a0 + 8u * ks, a_i = a0 + 16u + 8u * ks;
+                            ptx::mma_i8_ts<1>(0, a_i, dBr, idesc, acc);    // IR
+                            ptx::mma_i8_ts<1>(128, a_i, dBi, idesc, acc);  // II  -> Re
+                            ptx::mma_i8_ts<1>(256, a_r, dBi, idesc, acc);  // RI
+                            ptx::mma_i8_ts<1>(128, a_r, dBr, idesc, 1);    // RR  -> Re
+                            acc = 1;
+                        }
+                        ptx::mma_commit<1>(pl_empty(st));
+                    }
+                    __syncwarp();
+                }
+                ph ^= 1u;
+            }
+            if (issuer) ptx::mma_commit<1>(acc_full);
+            __syncwarp();
+            acc_ph ^= 1u;
+        }
+    } else if (warp < TD_EPI_WARP0) {
+        // ===================== S2: unpack =====================
+        // Two groups of four warps take the stages alternately: what a stage costs a warp is a chain of waits and
+        // latencies (barrier, ldmatrix, tcgen05.st, plane stores, fences, arrive) of more than the 512 cycles its MMAs
+        // take, so each group gets two stage times for it.  Both rings have an even number of stages and a unit an even
+        // number of stages: a ring position always belongs to the same group.  Warp <-> TMEM lane quarter q (hardware
+        // rule); it transposes both 32-sample halves of the stage for its 32 inputs.
+        static_assert(TD_PK_STAGES % 2 == 0 && TD_PL_STAGES % 2 == 0, "ring positions must keep their group");
+        const int q = warp & 3;
+        const int grp = (warp - 2) >> 2;        // parity of the stages this warp works on
+        const int gt = 32 * q + lane;           // thread of the group: 16-byte chunks gt + 128 c, c = 0..3
+        // ldmatrix row address of this lane, per half kh: matrix m = lane/16, row r = lane%16 -> sample 32 kh + 16 m + r
+        const int lrow = 16 * (lane >> 4) + (lane & 15);
+        const uint32_t lds0 = (uint32_t)lrow * 128u + ((uint32_t)((2 * q + 0) ^ (lrow & 7)) << 4);
+        const uint32_t lds1 = (uint32_t)lrow * 128u + ((uint32_t)((2 * q + 1) ^ (lrow & 7)) << 4);
+        const int tbase = 4 * (lane & 3);       // first sample of this thread's r0/r1 inside a half (r2/r3: + 16)
+        const uint32_t tdst = tmem + ((uint32_t)(32 * q) << 16) + TD_ACOL0;
+        int pst = grp, qst = grp;               // ring positions of this group's next stage
+        uint32_t pph = 0, qph = 0;
+        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+            int f, t_begin, t_end, ngroups;
+            unit(u, f, t_begin, t_end, ngroups);
+            for (int t = t_begin + grp * TD_ST; t < t_begin + ngroups * TD_GROUP; t += 2 * TD_ST) {
+                const int rows_valid = t_end - t;  // <= 0 in a padding stage: all-zero operands
+                ptx::mbar_wait(pk_full(pst), pph);
+                const uint32_t src = pk0 + pst * TD_PK_BYTES;
+                // ---- loads first: four transposing loads (rows' planes), four 16-byte chunks (columns' planes)
+                uint32_t xa[2][4], xb[2][4];
+#pragma unroll
+                for (int kh = 0; kh < 2; ++kh) {
+                    ptx::ldsm_t_b8_x2(src + 4096u * kh + lds0, xa[kh][0], xa[kh][1], xa[kh][2], xa[kh][3]);   // inputs 32q + 0..15
+                    ptx::ldsm_t_b8_x2(src + 4096u * kh + lds1, xb[kh][0], xb[kh][1], xb[kh][2], xb[kh][3]);   // inputs 32q + 16..31
+                }
+                uint4 wy[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) wy[c] = *reinterpret_cast<const uint4 *>(gbase + (src - base) + 2048 * c + gt * 16);
+                ptx::mbar_wait(pl_empty(qst), qph ^ 1u);
+                // ---- A planes -> TMEM
+#pragma unroll
+                for (int kh = 0; kh < 2; ++kh) {
+                    // byte masks of this thread's four samples (zero beyond the slice)
+                    uint32_t m0 = 0xF0F0F0F0u, m1 = 0xF0F0F0F0u;
+                    if (rows_valid < TD_ST) {
+                        const int v0 = min(4, max(0, rows_valid - 32 * kh - tbase)), v1 = min(4, max(0, rows_valid - 32 * kh - tbase - 16));
+                        m0 = v0 ? (0xF0F0F0F0u >> (32 - 8 * v0)) : 0u;
+                        m1 = v1 ? (0xF0F0F0F0u >> (32 - 8 * v1)) : 0u;
+                    }
+                    const uint32_t ta = tdst + (uint32_t)qst * TD_ACOLS + 8u * kh;
+                    ptx::tmem_st_16x128b_x2(ta, (xa[kh][0] ^ 0x80808080u) & m0, (xa[kh][1] ^ 0x80808080u) & m0,
+                                            (xa[kh][2] ^ 0x80808080u) & m1, (xa[kh][3] ^ 0x80808080u) & m1);
+                    ptx::tmem_st_16x128b_x2(ta + (16u << 16), (xb[kh][0] ^ 0x80808080u) & m0, (xb[kh][1] ^ 0x80808080u) & m0,
+                                            (xb[kh][2] ^ 0x80808080u) & m1, (xb[kh][3] ^ 0x80808080u) & m1);
+                    ptx::tmem_st_16x128b_x2(ta + 16u, ((xa[kh][0] << 4) ^ 0x80808080u) & m0, ((xa[kh][1] << 4) ^ 0x80808080u) & m0,
+                                            ((xa[kh][2] << 4) ^ 0x80808080u) & m1, ((xa[kh][3] << 4) ^ 0x80808080u) & m1);
+                    ptx::tmem_st_16x128b_x2(ta + (16u << 16) + 16u, ((xb[kh][0] << 4) ^ 0x80808080u) & m0,
+                                            ((xb[kh][1] << 4) ^ 0x80808080u) & m0, ((xb[kh][2] << 4) ^ 0x80808080u) & m1,
+                                            ((xb[kh][3] << 4) ^ 0x80808080u) & m1);
+                }
+                // ---- B planes -> shared memory, same physical offsets as the packed block (128-byte rows)
+                {
+                    uint8_t *dst = gbase + (pl0 - base) + qst * TD_PL_BYTES;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const uint32_t off = (uint32_t)gt * 16u + 2048u * c;
+                        const uint32_t m = ((int)(off >> 7) < rows_valid) ? 0xF0F0F0F0u : 0u;
+                        uint4 r, i;
+                        r.x = (wy[c].x ^ 0x80808080u) & m; r.y = (wy[c].y ^ 0x80808080u) & m;
+                        r.z = (wy[c].z ^ 0x80808080u) & m; r.w = (wy[c].w ^ 0x80808080u) & m;
+                        i.x = ((wy[c].x << 4) ^ 0x80808080u) & m; i.y = ((wy[c].y << 4) ^ 0x80808080u) & m;
+                        i.z = ((wy[c].z << 4) ^ 0x80808080u) & m; i.w = ((wy[c].w << 4) ^ 0x80808080u) & m;
+                        *reinterpret_cast<uint4 *>(dst + off) = r;
+                        *reinterpret_cast<uint4 *>(dst + TD_PLANE + off) = i;
+                    }
+                }
+                ptx::fence_proxy_async_smem();   // B planes: generic-proxy writes, read by the MMA's async proxy
+                ptx::tmem_st_wait();             // A planes are in TMEM
+                ptx::tc_fence_before_sync();
+                __syncwarp();
+                if (lane == 0) {
+                    ptx::mbar_arrive(pl_full(qst));
+                    ptx::mbar_arrive(pk_empty(pst));
+                }
+                pst += 2;
+                if (pst >= TD_PK_STAGES) { pst -= TD_PK_STAGES; pph ^= 1u; }
+                qst += 2;
+                if (qst >= TD_PL_STAGES) { qst -= TD_PL_STAGES; qph ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== S5: epilogue =====================
+        // Eight warps: warp % 4 = TMEM lane quarter q (hardware rule), h = column half.  Thread <-> row r = 32 q + lane of
+        // the tile, columns 64 h .. 64 h + 63.  The accumulators are drained into a shared-memory image of the row (8
+        // bytes per baseline, the layout of vis), TMEM is handed back as soon as the last tcgen05.ld has completed, and
+        // the row segment leaves as ONE bulk copy (cp.async.bulk, or cp.reduce.async.bulk.add.s32 when the call adds)
+        // that overlaps the next unit's main loop.  Rows of the packed triangle start on 8-byte boundaries and bulk
+        // copies need 16: the image is shifted by one slot when the global address is odd in 8-byte units, and at most
+        // one leading and one trailing baseline are written with ordinary stores.
+        const int q = warp & 3;
+        const int h = (warp - TD_EPI_WARP0) >> 2;
+        const int r = 32 * q + lane;                       // row of the tile
+        const int sub = p.sub;                             // 128, or 64: two channels per tile
+        const int cs = (sub == 64) ? (r >> 6) : 0;         // channel of the tile this row belongs to
+        const int xl = r - cs * sub;                       // input index inside its channel
+        const int cpt = 128 / sub;
+        const int img0 = (r < 64) ? 0 : 64;                // tile column held by slot `par` of this row's image
+        const uint32_t srow = epi0 + (r < 64 ? (uint32_t)r * TD_PITCH_LO : 64u * TD_PITCH_LO + (uint32_t)(r - 64) * TD_PITCH_HI);
+        uint8_t *srow_g = epi_g + (srow - epi0);
+        const long long Bn = (long long)p.n_out * ((long long)p.n_out + 1) / 2;
+        const bool add = (p.out_mode != OUT_STORE);
+        const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
+        uint32_t acc_ph = 0;
+        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+            int f, t_begin, t_end, ngroups;
+            unit(u, f, t_begin, t_end, ngroups);
+            // 8-byte index in vis of (this row, tile column img0) -- formal when that column is left of the diagonal:
+            // only its parity and offsets from it are used
+            const long long gi0 = (long long)(f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +
+                                  (img0 - cs * sub);
+            int2 *gimg = reinterpret_cast<int2 *>(p.vis) + gi0;
+            const uint32_t par = (uint32_t)(reinterpret_cast<uintptr_t>(gimg) >> 3) & 1u;
+            ptx::bulk_wait_read0();  // this thread's previous row segment has left shared memory
+            ptx::mbar_wait(acc_full, acc_ph);
+            acc_ph ^= 1u;
+            ptx::tc_fence_after_sync();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int col = 64 * h + 16 * c;
+                // warp-uniform: the chunk is left of the diagonal for every row of the warp, outside the matrix, or
+                // (two channels per tile) in the other channel's columns
+                const bool skip = (col + 15 < 32 * q) ||
+                                  (sub == 128 ? (col >= p.n_out || 32 * q >= p.n_out) : ((col >> 6) != (q >> 1)));
+                if (!skip) {
+                    uint32_t ir[16], rr[16], ri[16];
+                    ptx::tmem_ld16(trow + col, ir);
+                    ptx::tmem_ld16(trow + 128 + col, rr);
+                    ptx::tmem_ld16(trow + 256 + col, ri);
+                    ptx::tmem_ld_wait();
+                    uint8_t *dst = srow_g + 8 * ((int)par + col - img0);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int re = (int)rr[j] >> 8;
+                        const int im = (int)(ir[j] - ri[j]) >> 8;
+                        *reinterpret_cast<int2 *>(dst + j * 8) = make_int2(re, im);
+                    }
+                }
+            }
+            // TMEM is free for the next unit
+            ptx::tc_fence_before_sync();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(acc_empty);
+            // ---- the row segment [jlo, jhi) of tile columns this thread sends
+            int jlo = max(64 * h, r), jhi = min(64 * h + 64, cs * sub + p.n_out);
+            if (sub == 64 && h != cs) jhi = jlo;
+            if (xl < p.n_out && jlo < jhi) {
+                ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
+                int a = jlo - img0, b = jhi - img0;   // as offsets from the image's first column
+                if ((par + a) & 1) {             // leading baseline on an odd 8-byte slot
+                    const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * ((int)par + a));
+                    if (add) { atomicAdd(&gimg[a].x, v.x); atomicAdd(&gimg[a].y, v.y); }
+                    else gimg[a] = v;
+                    ++a;
+                }
+                if ((b - a) & 1) {               // trailing baseline
+                    --b;
+                    const int2 v = *reinterpret_cast<const int2 *>(srow_g + 8 * ((int)par + b));
+                    if (add) { atomicAdd(&gimg[b].x, v.x); atomicAdd(&gimg[b].y, v.y); }
+                    else gimg[b] = v;
+                }
+                if (a < b) {
+                    if (add) ptx::bulk_reduce_add_s32(gimg + a, srow + 8u * (par + a), 8u * (b - a));
+                    else ptx::bulk_store(gimg + a, srow + 8u * (par + a), 8u * (b - a));
+                }
+            }
+            ptx::bulk_commit();
+        }
+        ptx::bulk_wait0();  // every row segment has been written before the CTA retires
+    }
+
+    __syncwarp();  // lanes that skipped the single-thread roles rejoin here
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc<1>(tmem, 512);
+}
+
+}  // namespace corr

@@ -199,6 +199,27 @@ def test_n64_two_channels_per_tile(corr, oracle, F):
         assert np.array_equal(got, oracle.level1(packed)), (F, hex(byte))
 
 
+@pytest.mark.parametrize("shape", [(128, 3, 1000), (128, 1, 70000), (128, 310, 300), (112, 2, 257), (100, 5, 4099),
+                                   (96, 2, 64), (17, 3, 900), (128, 2, 1), (65, 4, 33000)])
+def test_diagonal_block_kernel(corr, oracle, shape):
+    # N <= 128 on the tcgen05 path is one 128-block per channel: corr_tcd_kernel (A operand in TMEM, two groups of
+    # unpack warps, row images of the upper triangle sent as bulk copies).  Ragged N (also N % 16 != 0 through the padded
+    # stream) and T, T split into slices of whole groups of 256 samples, more units than SMs, stale output, accumulation
+    N, F, T = shape
+    packed = workloads.uniform_bytes(N, F, T, seed=N * 7 + F + T)
+    want = oracle.level1(packed)
+    got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=-559038737)
+    assert info["path"] == corr.PATH_TCGEN05 and info["tiles_per_channel"] == 1
+    assert np.array_equal(got, want), shape
+    again, _ = _run(corr, packed, corr.PATH_TCGEN05, accumulate_into=got.copy())
+    assert np.array_equal(again, 2 * want), (shape, "accumulate")
+    if T >= 900:
+        for byte in (0x00, 0xFF, 0x0F, 0xF0):                  # largest magnitudes everywhere
+            packed = np.full((min(T, 5000), min(F, 3), N), byte, np.uint8)
+            got, _ = _run(corr, packed, corr.PATH_TCGEN05)
+            assert np.array_equal(got, oracle.level1(packed)), (shape, hex(byte))
+
+
 @pytest.mark.parametrize("variant", ["1", "3", "5"])
 def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
     # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles (automatic for N <= 128), 3 CTA pair
