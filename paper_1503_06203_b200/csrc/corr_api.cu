@@ -174,6 +174,7 @@ struct corr_plan {
                        // for N <= 128, where a pair tile would be half empty, and for two 64-input channels per tile);
                        // 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default above N = 128);
                        // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
+    int balanced;      // variant 2: all groups of all channels dealt to the CTAs in equal shares (corr_tcd.cuh), output added
     int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
     long long total_groups;
     int *flags_dev;    // variant 3: [num_units][2] stream-K flags (corr_tc3.cuh)
@@ -496,6 +497,23 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
     p->grid = (path == CORR_PATH_DP4A) ? p->num_units
               : (p->variant >= 3) ? 2 * std::min(p->num_units, p->sm_count / 2)
                                   : std::min(p->num_units, p->sm_count);
+    if (p->variant == 2) {
+        // few, long channels leave SMs idle (64 channels in two slices: 128 units for 148 SMs): deal the groups of 256
+        // samples of all channels to the CTAs in equal shares instead, every share added into a cleared output
+        const long long gpc = (T + corr::TD_GROUP - 1) / corr::TD_GROUP, G = units0 * gpc;
+        const long long waves = (p->num_units + p->sm_count - 1) / p->sm_count;
+        const double extra = 512.0;   // samples' worth of time per segment: accumulator drain, epilogue, pipeline restart
+        const double simple_cost = (double)waves * (p->t_per_slice + extra);
+        const double shares_cost = (double)((G + p->sm_count - 1) / p->sm_count) * corr::TD_GROUP + 3.0 * extra;
+        const char *e = getenv("CORR_TCD_SHARES");   // testing aid: 0 / 1 forces the choice
+        // equal shares put the CTAs at 148 different times of the stream (units of a wave sweep it together), which costs
+        // DRAM locality: measured, the shares win by 5 - 9 % at 128-byte rows (N = 128, two channels of 64) for a 6 % better
+        // fill and lose 8 % at N = 112, so rows that are not 128 bytes need a clear gain (N = 96, F = 100: + 13 % for 18 %)
+        const double need = (n_pad == 128 || packed64) ? 0.97 : 0.85;
+        p->balanced = (G >= p->sm_count && shares_cost < need * simple_cost) ? 1 : 0;
+        if (e && G >= 1) p->balanced = (e[0] != '0') ? 1 : 0;
+        if (p->balanced) p->grid = (int)std::min<long long>(G, p->sm_count);
+    }
     p->kernels_per_exec = 1 + ((path != CORR_PATH_DP4A && n_pad != N) ? 1 : 0);  // + corr_pad_kernel
     p->aligned = (N % 4 == 0) ? 1 : 0;
     if (p->variant >= 3) {
@@ -709,7 +727,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         packed_dev = p->pad_buf;
     }
     int out_mode;
-    if (p->slices > 1) {
+    if (p->slices > 1 || p->balanced) {
         out_mode = corr::OUT_ATOMIC;
         if (!accumulate_flag)
             CUDA_TRY(cudaMemsetAsync(vis_dev, 0, corr_vis_elems(p) * sizeof(int32_t), stream), CORR_ERR_CUDA);
@@ -799,7 +817,8 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.n_out = p->N;
             prm.T = p->T;
             prm.tiles_per_f = p->tiles_per_f;
-            prm.slices = p->slices;
+            prm.slices = p->balanced ? 0 : p->slices;
+            prm.groups_per_f = (p->T + corr::TD_GROUP - 1) / corr::TD_GROUP;
             prm.t_per_slice = p->t_per_slice;
             prm.num_units = p->num_units;
             prm.out_mode = out_mode;

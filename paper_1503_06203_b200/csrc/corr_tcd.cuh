@@ -102,14 +102,42 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     const uint32_t tmem = *tmem_slot_g;
     if (tmem != 0) __trap();  // all 512 columns were requested: the allocation starts at lane 0, column 0
 
-    // unit u = (channel f, T-slice): samples [t_begin, t_end), run as whole groups of TD_GROUP samples (the stages
-    // beyond t_end are loaded -- TMA fills rows beyond T with zeros -- and masked to zero operands by the unpack)
-    auto unit = [&](int u, int &f, int &t_begin, int &t_end, int &ngroups) {
-        f = u / p.slices;
-        const int slice = u - f * p.slices;
-        t_begin = slice * p.t_per_slice;
-        t_end = min(p.T, t_begin + p.t_per_slice);
-        ngroups = (t_end - t_begin + TD_GROUP - 1) / TD_GROUP;
+    // The work of a call is cut into SEGMENTS (channel f, samples [t_begin, t_end)), each run as whole groups of TD_GROUP
+    // samples (the stages beyond t_end are loaded -- TMA fills rows beyond T with zeros -- and masked to zero operands
+    // by the unpack).  Two schedules, chosen by the host:
+    //   slices > 0   unit u = (channel, T-slice), units dealt round-robin: every channel's sum has one owner (or a few
+    //                when T is split for int32 headroom or to fill the SMs);
+    //   slices == 0  all groups of all channels in one row, cut into gridDim.x EQUAL shares: a CTA's share covers
+    //                parts of up to a few channels, every segment is added into vis (which the host has cleared).
+    //                This is what fills 148 SMs when the channels are few and long (64 channels: 128 units otherwise).
+    long long it, it_end;
+    if (p.slices > 0) {
+        it = blockIdx.x;
+        it_end = p.num_units;
+    } else {
+        const long long G = (long long)p.F * p.groups_per_f;
+        it = G * blockIdx.x / gridDim.x;
+        it_end = G * (blockIdx.x + 1) / gridDim.x;
+    }
+    auto next_segment = [&](int &f, int &t_begin, int &t_end, int &ngroups) -> bool {
+        if (it >= it_end) return false;
+        if (p.slices > 0) {
+            const int u = (int)it;
+            f = u / p.slices;
+            const int slice = u - f * p.slices;
+            t_begin = slice * p.t_per_slice;
+            t_end = min(p.T, t_begin + p.t_per_slice);
+            ngroups = (t_end - t_begin + TD_GROUP - 1) / TD_GROUP;
+            it += gridDim.x;
+        } else {
+            f = (int)(it / p.groups_per_f);
+            const int first = (int)(it - (long long)f * p.groups_per_f);
+            ngroups = (int)min((long long)min(p.groups_per_f - first, TD_MAX_SLICE / TD_GROUP), it_end - it);
+            t_begin = first * TD_GROUP;
+            t_end = min(p.T, t_begin + ngroups * TD_GROUP);
+            it += ngroups;
+        }
+        return true;
     };
 
     if (warp == 0) {
@@ -117,9 +145,9 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         if (lane == 0) {
             int st = 0;
             uint32_t ph = 0;
-            for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+            for (;;) {
                 int f, t_begin, t_end, ngroups;
-                unit(u, f, t_begin, t_end, ngroups);
+                if (!next_segment(f, t_begin, t_end, ngroups)) break;
                 for (int t = t_begin; t < t_begin + ngroups * TD_GROUP; t += TD_ST) {
                     ptx::mbar_wait(pk_empty(st), ph ^ 1u);
                     ptx::mbar_arrive_expect_tx(pk_full(st), TD_PK_BYTES);
@@ -134,9 +162,9 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         constexpr uint32_t idesc = make_idesc_i8(128, 128, true, true, /*A K-major (TMEM)*/ false, /*B MN-major*/ true);
         uint32_t ph = 0, acc_ph = 0;
         const bool issuer = ptx::elect_one();
-        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+        for (;;) {
             int f, t_begin, t_end, ngroups;
-            unit(u, f, t_begin, t_end, ngroups);
+            if (!next_segment(f, t_begin, t_end, ngroups)) break;
             ptx::mbar_wait(acc_empty, acc_ph ^ 1u);
             ptx::tc_fence_after_sync();
             uint32_t acc = 0;
@@ -189,9 +217,9 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const uint32_t tdst = tmem + ((uint32_t)(32 * q) << 16) + TD_ACOL0;
         int pst = grp, qst = grp;               // ring positions of this group's next stage
         uint32_t pph = 0, qph = 0;
-        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+        for (;;) {
             int f, t_begin, t_end, ngroups;
-            unit(u, f, t_begin, t_end, ngroups);
+            if (!next_segment(f, t_begin, t_end, ngroups)) break;
             for (int t = t_begin + grp * TD_ST; t < t_begin + ngroups * TD_GROUP; t += 2 * TD_ST) {
                 const int rows_valid = t_end - t;  // <= 0 in a padding stage: all-zero operands
                 ptx::mbar_wait(pk_full(pst), pph);
@@ -281,9 +309,9 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const bool add = (p.out_mode != OUT_STORE);
         const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
         uint32_t acc_ph = 0;
-        for (int u = blockIdx.x; u < p.num_units; u += gridDim.x) {
+        for (;;) {
             int f, t_begin, t_end, ngroups;
-            unit(u, f, t_begin, t_end, ngroups);
+            if (!next_segment(f, t_begin, t_end, ngroups)) break;
             // 8-byte index in vis of (this row, tile column img0) -- formal when that column is left of the diagonal:
             // only its parity and offsets from it are used
             const long long gi0 = (long long)(f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +

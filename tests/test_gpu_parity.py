@@ -201,10 +201,15 @@ def test_n64_two_channels_per_tile(corr, oracle, F):
 
 @pytest.mark.parametrize("shape", [(128, 3, 1000), (128, 1, 70000), (128, 310, 300), (112, 2, 257), (100, 5, 4099),
                                    (96, 2, 64), (17, 3, 900), (128, 2, 1), (65, 4, 33000)])
-def test_diagonal_block_kernel(corr, oracle, shape):
+@pytest.mark.parametrize("shares", ["auto", "1", "0"])
+def test_diagonal_block_kernel(corr, oracle, shape, shares, monkeypatch):
     # N <= 128 on the tcgen05 path is one 128-block per channel: corr_tcd_kernel (A operand in TMEM, two groups of
     # unpack warps, row images of the upper triangle sent as bulk copies).  Ragged N (also N % 16 != 0 through the padded
-    # stream) and T, T split into slices of whole groups of 256 samples, more units than SMs, stale output, accumulation
+    # stream) and T, T split into slices of whole groups of 256 samples, more units than SMs, stale output, accumulation.
+    # Both schedules: units (channel, T-slice) dealt round-robin, and equal shares of all groups of all channels added
+    # into a cleared output (CORR_TCD_SHARES forces one; the plan chooses by a cost model otherwise)
+    if shares != "auto":
+        monkeypatch.setenv("CORR_TCD_SHARES", shares)
     N, F, T = shape
     packed = workloads.uniform_bytes(N, F, T, seed=N * 7 + F + T)
     want = oracle.level1(packed)
