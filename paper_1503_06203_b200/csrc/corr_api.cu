@@ -506,10 +506,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         const double simple_cost = (double)waves * (p->t_per_slice + extra);
         const double shares_cost = (double)((G + p->sm_count - 1) / p->sm_count) * corr::TD_GROUP + 3.0 * extra;
         const char *e = getenv("CORR_TCD_SHARES");   // testing aid: 0 / 1 forces the choice
-        // equal shares put the CTAs at 148 different times of the stream (units of a wave sweep it together), which costs
-        // DRAM locality: measured, the shares win by 5 - 9 % at 128-byte rows (N = 128, two channels of 64) for a 6 % better
-        // fill and lose 8 % at N = 112, so rows that are not 128 bytes need a clear gain (N = 96, F = 100: + 13 % for 18 %)
-        const double need = (n_pad == 128 || packed64) ? 0.97 : 0.85;
+        // (equal shares put the CTAs at 148 different times of the stream, where units of a wave sweep it together: the
+        // tensor map of this schedule asks for 64-byte L2 promotion instead of 256, see build_tmap)
+        const double need = 0.97;
         p->balanced = (G >= p->sm_count && shares_cost < need * simple_cost) ? 1 : 0;
         if (e && G >= 1) p->balanced = (e[0] != '0') ? 1 : 0;
         if (p->balanced) p->grid = (int)std::min<long long>(G, p->sm_count);
@@ -689,9 +688,16 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const int st = (p->variant >= 3) ? corr::T3_ST : corr::TC_ST;
     const cuuint32_t box[3] = {128u, 1u, (cuuint32_t)st};
+    // L2 promotion: 256-byte lines pay when the neighbouring 128 bytes (the next channel's block at the same sample) are
+    // wanted soon, which is so when the CTAs sweep the stream together; the equal-shares schedule of corr_tcd_kernel
+    // puts them at 148 different times (ncu: 402 MB read from DRAM for a 268 MB stream with 256-byte promotion; measured
+    // with 256 / 128 / 64 bytes / none: 86.2 / 83.1 / 83.0 / 83.2 us at N = 128, F = 64 and 101.0 / 90.6 / 86.5 / 90.6 at N = 112)
+    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
+    if (p->variant == 2 && p->balanced) promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
+    if (const char *e = getenv("CORR_TCD_PROMO")) promo = (atoi(e) == 128) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : (atoi(e) == 64) ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : (atoi(e) == 0) ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                 promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r == CUDA_SUCCESS && p->variant >= 3) {
         const cuuint32_t boxy[3] = {64u, 1u, (cuuint32_t)st};  // half a y-block per CTA of the pair
         r = get_encode_fn()(&p->tmap_y, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
