@@ -694,7 +694,6 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
     // with 256 / 128 / 64 bytes / none: 86.2 / 83.1 / 83.0 / 83.2 us at N = 128, F = 64 and 101.0 / 90.6 / 86.5 / 90.6 at N = 112)
     CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
     if (p->variant == 2 && p->balanced) promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
-    if (const char *e = getenv("CORR_TCD_PROMO")) promo = (atoi(e) == 128) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : (atoi(e) == 64) ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : (atoi(e) == 0) ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
     CUresult r = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(packed_dev), dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                  promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
