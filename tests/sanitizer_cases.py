@@ -66,8 +66,8 @@ def cases(s0):
     # corr_tc5_kernel: the same schedule, per-element sums through shared memory of both CTAs of the pair
     ok &= run("tc5 cut units", workloads.uniform_bytes(256, 2, 20000, seed=s0 + 4), corr.PATH_TCGEN05, "5", accumulate=True)
     ok &= run("tc5 transposed tiles, ragged N and T", workloads.uniform_bytes(400, 2, 777, seed=s0 + 5), corr.PATH_TCGEN05, "5")
-    # corr_tc_kernel: single-CTA tiles (N <= 128), padded stream
-    ok &= run("tc single-CTA tiles", workloads.uniform_bytes(100, 3, 3000, seed=s0 + 6), corr.PATH_TCGEN05, None)
+    # corr_tcd_kernel: one CTA per channel's block (N <= 128), padded stream
+    ok &= run("tcd one block per channel", workloads.uniform_bytes(100, 3, 3000, seed=s0 + 6), corr.PATH_TCGEN05, None)
     # corr_imma_kernel: several chunks per strip (shared-memory atomics, global atomics)
     ok &= run("imma several chunks", workloads.uniform_bytes(32, 9, 4099, seed=s0 + 7), corr.PATH_IMMA)
     ok &= run("dp4a", workloads.uniform_bytes(17, 3, 650, seed=s0 + 8), corr.PATH_DP4A)

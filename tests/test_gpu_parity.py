@@ -182,7 +182,7 @@ def test_determinism(corr):
 
 @pytest.mark.parametrize("F", [2, 6, 16, 3])
 def test_n64_two_channels_per_tile(corr, oracle, F):
-    # N = 64, even F: AUTO runs single-CTA tcgen05 tiles on the stream seen as [T][F/2][128] and writes the two
+    # N = 64, even F: AUTO runs corr_tcd_kernel (one CTA per 128-block) on the stream seen as [T][F/2][128] and writes the two
     # diagonal 64-blocks of each tile as channels 2f, 2f + 1; odd F stays on the warp-MMA kernel.  Ragged T, split T,
     # stale output, accumulation, extreme bytes.
     for T in (1, 63, 300, 4099, 70000 if F == 2 else 1000):
@@ -227,7 +227,7 @@ def test_diagonal_block_kernel(corr, oracle, shape, shares, monkeypatch):
 
 @pytest.mark.parametrize("variant", ["1", "3", "5"])
 def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
-    # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles (automatic for N <= 128), 3 CTA pair
+    # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles with both operands in shared memory (round 1's kernel; N <= 128 runs corr_tcd_kernel unless this forces it), 3 CTA pair
     # with the A operand in TMEM (automatic above), 5 three products per complex MAC on the stored bytes with
     # fused per-element sums (offset route, Eq. 3).  Same bits from all of them, including ragged N (also
     # N % 16 != 0 through the padded stream), split T, cut units and accumulation.
