@@ -444,7 +444,21 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         p->variant = (v && !strcmp(v, "1")) ? 1 : (v && !strcmp(v, "3")) ? 3 : (v && !strcmp(v, "5")) ? 5 : (n_pad <= 128) ? 1 : 3;
         if (packed64) p->variant = 1;
         // one 128-block per channel: the diagonal-block kernel (A operand in TMEM, corr_tcd.cuh) unless variant 1 is forced
-        if (p->variant == 1 && (packed64 || n_pad <= 128) && !(v && !strcmp(v, "1"))) p->variant = 2;
+        // Two or three blocks per channel (128 < N <= 256): the same kernel with off-diagonal blocks (two packed blocks per
+        // stage, the image used by the two halves of a block in turn) beats the pair kernel, which computes one of its two
+        // pair tiles next to an empty block there, when the segments are long: measured N = 256: 2384 against 1978 TOPS
+        // at F = 32, T = 32768 and 41.5 against 44.7 us on cfg 2, but 53.7 against 49.9 us at F = 128, T = 2048 (segments of
+        // 8 groups) and above N = 256 the pair kernel wins (N = 272: 1225 against 1455).  CORR_TCD_MAX_N (testing aid)
+        // moves the upper limit.
+        const char *mx = getenv("CORR_TCD_MAX_N");
+        const int tcd_max = mx ? atoi(mx) : 256;
+        {
+            const long long nbk = (n_pad + 127) / 128, gpc = (T + corr::TD_GROUP - 1) / corr::TD_GROUP;
+            const long long G = (long long)F * (nbk * (nbk + 1) / 2) * gpc;
+            const double seg = std::min<double>((double)gpc, (double)G / (double)std::min<long long>(G, p->sm_count));
+            if (!(v && v[0]) && !packed64 && n_pad > 128 && n_pad <= tcd_max && (seg >= 16.0 || mx)) p->variant = 1;
+        }
+        if (p->variant == 1 && (packed64 || n_pad <= std::max(128, tcd_max)) && !(v && !strcmp(v, "1"))) p->variant = 2;
     }
     p->pack_sub = packed64 ? 64 : 128;
     const int Ns = packed64 ? 128 : N, Fs = packed64 ? F / 2 : F;   // the shape the tile schedule sees
@@ -556,7 +570,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         cudaError_t e5 = cudaFuncSetAttribute(corr::corr_tc5_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               corr::T5_SMEM_BYTES);
         if (e5 == cudaSuccess)
-            e5 = cudaFuncSetAttribute(corr::corr_tcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::TD_SMEM_BYTES);
+            e5 = cudaFuncSetAttribute(corr::corr_tcd_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::TD_SMEM_BYTES);
+        if (e5 == cudaSuccess)
+            e5 = cudaFuncSetAttribute(corr::corr_tcd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, corr::TD_SMEM_BYTES_G);
         if (e1 != cudaSuccess || e3 != cudaSuccess || e5 != cudaSuccess) {
             g_create_rc = CORR_ERR_CUDA; set_err("corr_plan_create: cannot reserve %d / %d / %d B of shared memory: %s", corr::TC_SMEM_BYTES,
                     corr::T3_SMEM_BYTES, corr::T5_SMEM_BYTES, cudaGetErrorString(cudaGetLastError()));
@@ -829,8 +845,10 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.out_mode = out_mode;
             prm.tiles = p->tiles_dev;
             prm.vis = vis_dev;
-            if (p->variant == 2)
-                corr::corr_tcd_kernel<<<p->grid, corr::TD_THREADS, corr::TD_SMEM_BYTES, stream>>>(p->tmap, prm);
+            if (p->variant == 2 && p->tiles_per_f > 1)
+                corr::corr_tcd_kernel<true><<<p->grid, corr::TD_THREADS, corr::TD_SMEM_BYTES_G, stream>>>(p->tmap, prm);
+            else if (p->variant == 2)
+                corr::corr_tcd_kernel<false><<<p->grid, corr::TD_THREADS, corr::TD_SMEM_BYTES, stream>>>(p->tmap, prm);
             else
                 corr::corr_tc_kernel<<<p->grid, corr::TC_THREADS, corr::TC_SMEM_BYTES, stream>>>(p->tmap, prm);
         }

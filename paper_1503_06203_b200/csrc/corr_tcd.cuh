@@ -39,7 +39,8 @@ constexpr int TD_ST = 64;               // time samples per stage
 #ifndef TD_PL_N
 #define TD_PL_N 4
 #endif
-constexpr int TD_PK_STAGES = TD_PK_N;   // packed-byte ring
+constexpr int TD_PK_STAGES = TD_PK_N;   // packed-byte ring when every tile is a diagonal block (N <= 128): one block per stage
+constexpr int TD_PK_STAGES_G = 6;       // ... when the triangle has off-diagonal blocks: rows' block + columns' block per stage
 constexpr int TD_PL_STAGES = TD_PL_N;   // operand ring: TMEM A stage + smem B stage
 constexpr int TD_GROUP = TD_ST * TD_PL_STAGES;   // a unit runs whole groups of stages (static ring positions in the MMA loop)
 constexpr int TD_UNPACK_WARPS = 8;
@@ -52,26 +53,39 @@ constexpr int TD_PL_BYTES = 2 * TD_PLANE;         // Br, Bi
 constexpr int TD_PITCH_LO = 128 * 8 + 16;         // image of a row 0..63: 128 baselines + parity slot
 constexpr int TD_PITCH_HI = 64 * 8 + 16;          // image of a row 64..127: columns 64..127 + parity slot
 constexpr int TD_EPI_BYTES = 64 * (TD_PITCH_LO + TD_PITCH_HI);
-constexpr int TD_SMEM_BYTES = 1024 + TD_PK_STAGES * TD_PK_BYTES + TD_PL_STAGES * TD_PL_BYTES + TD_EPI_BYTES + 256;
+constexpr int TD_SMEM_BYTES = 1024 + TD_PK_STAGES * TD_PK_BYTES + TD_PL_STAGES * TD_PL_BYTES + TD_EPI_BYTES + 384;
+// with off-diagonal blocks: a ring of double stages, and an image of 64 rows that the two halves of the block use in turn
+constexpr int TD_EPI_BYTES_G = 64 * TD_PITCH_LO;
+constexpr int TD_SMEM_BYTES_G = 1024 + TD_PK_STAGES_G * 2 * TD_PK_BYTES + TD_PL_STAGES * TD_PL_BYTES + TD_EPI_BYTES_G + 384;
+static_assert(TD_SMEM_BYTES <= 232448 && TD_SMEM_BYTES_G <= 232448, "227 KB of shared memory per CTA");
 constexpr uint32_t TD_ACOL0 = 384, TD_ACOLS = 32;
 constexpr int TD_MAX_SLICE = 32768;               // |sum| <= 2 * 128 * 128 * slice < 2^31
 
+// GENERAL = false: every tile is the diagonal block (0, 0) of its channel (N <= 128, or two channels of 64 per tile).
+// GENERAL = true: tiles (bx <= by) of p.tiles; off-diagonal tiles load two packed blocks per stage (rows', columns') into a
+// ring of TD_PK_STAGES_G double stages and write all 128 x 128 baselines.
+template <bool GENERAL>
 __global__ void __launch_bounds__(TD_THREADS, 1)
 corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 {
+    constexpr int PK_STAGES = GENERAL ? TD_PK_STAGES_G : TD_PK_STAGES;
+    constexpr int PK_BYTES = GENERAL ? 2 * TD_PK_BYTES : TD_PK_BYTES;
+    // a (ring position, unpack group) pair of barriers is used once every PK_PERIOD stages (stage j: position j % PK_STAGES,
+    // group j & 1; with an odd ring a group comes back to a position only every second time round)
+    constexpr int PK_PERIOD = (PK_STAGES % 2 == 0) ? PK_STAGES : 2 * PK_STAGES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - ptx::smem_u32(smem_raw));
     const uint32_t pk0 = base;
-    const uint32_t pl0 = pk0 + TD_PK_STAGES * TD_PK_BYTES;
+    const uint32_t pl0 = pk0 + PK_STAGES * PK_BYTES;
     const uint32_t epi0 = pl0 + TD_PL_STAGES * TD_PL_BYTES;
-    const uint32_t bar0 = epi0 + TD_EPI_BYTES;
+    const uint32_t bar0 = epi0 + (GENERAL ? TD_EPI_BYTES_G : TD_EPI_BYTES);
     uint8_t *epi_g = gbase + (epi0 - base);
-    auto pk_full = [&](int s) { return bar0 + 8u * s; };
-    auto pk_empty = [&](int s) { return bar0 + 8u * (TD_PK_STAGES + s); };
-    auto pl_full = [&](int s) { return bar0 + 8u * (2 * TD_PK_STAGES + s); };
-    auto pl_empty = [&](int s) { return bar0 + 8u * (2 * TD_PK_STAGES + TD_PL_STAGES + s); };
-    const uint32_t acc_full = bar0 + 8u * (2 * TD_PK_STAGES + 2 * TD_PL_STAGES);
+    auto pk_full = [&](int s, int g) { return bar0 + 8u * (2 * s + g); };
+    auto pk_empty = [&](int s, int g) { return bar0 + 8u * (2 * PK_STAGES + 2 * s + g); };
+    auto pl_full = [&](int s) { return bar0 + 8u * (4 * PK_STAGES + s); };
+    auto pl_empty = [&](int s) { return bar0 + 8u * (4 * PK_STAGES + TD_PL_STAGES + s); };
+    const uint32_t acc_full = bar0 + 8u * (4 * PK_STAGES + 2 * TD_PL_STAGES);
     const uint32_t acc_empty = acc_full + 8u;
     const uint32_t tmem_slot = acc_empty + 8u;
     volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + (tmem_slot - base));
@@ -80,10 +94,11 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tmap(&tmap);
-        for (int s = 0; s < TD_PK_STAGES; ++s) {
-            ptx::mbar_init(pk_full(s), 1);
-            ptx::mbar_init(pk_empty(s), TD_UNPACK_WARPS / 2);   // the group of unpack warps that owns the position
-        }
+        for (int s = 0; s < PK_STAGES; ++s)
+            for (int g = 0; g < 2; ++g) {
+                ptx::mbar_init(pk_full(s, g), 1);
+                ptx::mbar_init(pk_empty(s, g), TD_UNPACK_WARPS / 2);   // the group of unpack warps that takes the stage
+            }
         for (int s = 0; s < TD_PL_STAGES; ++s) {
             ptx::mbar_init(pl_full(s), TD_UNPACK_WARPS / 2);
             ptx::mbar_init(pl_empty(s), 1);
@@ -111,48 +126,64 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     //                parts of up to a few channels, every segment is added into vis (which the host has cleared).
     //                This is what fills 148 SMs when the channels are few and long (64 channels: 128 units otherwise).
     long long it, it_end;
+    const int tiles_per_f = GENERAL ? p.tiles_per_f : 1;
     if (p.slices > 0) {
         it = blockIdx.x;
         it_end = p.num_units;
     } else {
-        const long long G = (long long)p.F * p.groups_per_f;
+        const long long G = (long long)p.F * tiles_per_f * p.groups_per_f;
         it = G * blockIdx.x / gridDim.x;
         it_end = G * (blockIdx.x + 1) / gridDim.x;
     }
-    auto next_segment = [&](int &f, int &t_begin, int &t_end, int &ngroups) -> bool {
+    struct Seg { int f, bx, by, t_begin, t_end, ngroups; };
+    auto next_segment = [&](Seg &sg) -> bool {
         if (it >= it_end) return false;
+        int ft;   // (channel, tile)
         if (p.slices > 0) {
             const int u = (int)it;
-            f = u / p.slices;
-            const int slice = u - f * p.slices;
-            t_begin = slice * p.t_per_slice;
-            t_end = min(p.T, t_begin + p.t_per_slice);
-            ngroups = (t_end - t_begin + TD_GROUP - 1) / TD_GROUP;
+            ft = u / p.slices;
+            const int slice = u - ft * p.slices;
+            sg.t_begin = slice * p.t_per_slice;
+            sg.t_end = min(p.T, sg.t_begin + p.t_per_slice);
+            sg.ngroups = (sg.t_end - sg.t_begin + TD_GROUP - 1) / TD_GROUP;
             it += gridDim.x;
         } else {
-            f = (int)(it / p.groups_per_f);
-            const int first = (int)(it - (long long)f * p.groups_per_f);
-            ngroups = (int)min((long long)min(p.groups_per_f - first, TD_MAX_SLICE / TD_GROUP), it_end - it);
-            t_begin = first * TD_GROUP;
-            t_end = min(p.T, t_begin + ngroups * TD_GROUP);
-            it += ngroups;
+            ft = (int)(it / p.groups_per_f);
+            const int first = (int)(it - (long long)ft * p.groups_per_f);
+            sg.ngroups = (int)min((long long)min(p.groups_per_f - first, TD_MAX_SLICE / TD_GROUP), it_end - it);
+            sg.t_begin = first * TD_GROUP;
+            sg.t_end = min(p.T, sg.t_begin + sg.ngroups * TD_GROUP);
+            it += sg.ngroups;
+        }
+        sg.f = ft / tiles_per_f;
+        sg.bx = sg.by = 0;
+        if (GENERAL) {
+            const ushort2 tile = p.tiles[ft - sg.f * tiles_per_f];
+            sg.bx = tile.x;
+            sg.by = tile.y;
         }
         return true;
     };
+    Seg sg;
 
     if (warp == 0) {
         // ===================== S1: TMA producer =====================
         if (lane == 0) {
             int st = 0;
-            uint32_t ph = 0;
-            for (;;) {
-                int f, t_begin, t_end, ngroups;
-                if (!next_segment(f, t_begin, t_end, ngroups)) break;
-                for (int t = t_begin; t < t_begin + ngroups * TD_GROUP; t += TD_ST) {
-                    ptx::mbar_wait(pk_empty(st), ph ^ 1u);
-                    ptx::mbar_arrive_expect_tx(pk_full(st), TD_PK_BYTES);
-                    ptx::tma_load_3d(pk0 + st * TD_PK_BYTES, &tmap, pk_full(st), 0, f, t);
-                    if (++st == TD_PK_STAGES) { st = 0; ph ^= 1u; }
+            uint32_t j = 0;   // stages loaded so far: stage j goes to ring position j % PK_STAGES and to unpack group j & 1
+            while (next_segment(sg)) {
+                const bool diag = sg.bx == sg.by;
+                for (int t = sg.t_begin; t < sg.t_begin + sg.ngroups * TD_GROUP; t += TD_ST) {
+                    const int g = (int)(j & 1u);
+                    if (j >= (uint32_t)PK_STAGES) {   // the position's last stage, j - PK_STAGES, has been unpacked
+                        const uint32_t jp = j - PK_STAGES;
+                        ptx::mbar_wait(pk_empty(st, (int)(jp & 1u)), (jp / PK_PERIOD) & 1u);
+                    }
+                    ptx::mbar_arrive_expect_tx(pk_full(st, g), (!GENERAL || diag) ? TD_PK_BYTES : 2 * TD_PK_BYTES);
+                    ptx::tma_load_3d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), sg.bx * 128, sg.f, t);
+                    if (GENERAL && !diag) ptx::tma_load_3d(pk0 + st * PK_BYTES + TD_PK_BYTES, &tmap, pk_full(st, g), sg.by * 128, sg.f, t);
+                    ++j;
+                    if (++st == PK_STAGES) st = 0;
                 }
             }
         }
@@ -162,13 +193,11 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         constexpr uint32_t idesc = make_idesc_i8(128, 128, true, true, /*A K-major (TMEM)*/ false, /*B MN-major*/ true);
         uint32_t ph = 0, acc_ph = 0;
         const bool issuer = ptx::elect_one();
-        for (;;) {
-            int f, t_begin, t_end, ngroups;
-            if (!next_segment(f, t_begin, t_end, ngroups)) break;
+        while (next_segment(sg)) {
             ptx::mbar_wait(acc_empty, acc_ph ^ 1u);
             ptx::tc_fence_after_sync();
             uint32_t acc = 0;
-            for (int g = 0; g < ngroups; ++g) {
+            for (int g = 0; g < sg.ngroups; ++g) {
 #pragma unroll
                 for (int st = 0; st < TD_PL_STAGES; ++st) {
                     ptx::mbar_wait(pl_full(st), ph);
@@ -205,7 +234,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // take, so each group gets two stage times for it.  Both rings have an even number of stages and a unit an even
         // number of stages: a ring position always belongs to the same group.  Warp <-> TMEM lane quarter q (hardware
         // rule); it transposes both 32-sample halves of the stage for its 32 inputs.
-        static_assert(TD_PK_STAGES % 2 == 0 && TD_PL_STAGES % 2 == 0, "ring positions must keep their group");
+        static_assert(TD_PL_STAGES % 2 == 0, "operand ring positions must keep their group");
         const int q = warp & 3;
         const int grp = (warp - 2) >> 2;        // parity of the stages this warp works on
         const int gt = 32 * q + lane;           // thread of the group: 16-byte chunks gt + 128 c, c = 0..3
@@ -215,15 +244,15 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const uint32_t lds1 = (uint32_t)lrow * 128u + ((uint32_t)((2 * q + 1) ^ (lrow & 7)) << 4);
         const int tbase = 4 * (lane & 3);       // first sample of this thread's r0/r1 inside a half (r2/r3: + 16)
         const uint32_t tdst = tmem + ((uint32_t)(32 * q) << 16) + TD_ACOL0;
-        int pst = grp, qst = grp;               // ring positions of this group's next stage
-        uint32_t pph = 0, qph = 0;
-        for (;;) {
-            int f, t_begin, t_end, ngroups;
-            if (!next_segment(f, t_begin, t_end, ngroups)) break;
-            for (int t = t_begin + grp * TD_ST; t < t_begin + ngroups * TD_GROUP; t += 2 * TD_ST) {
+        int pst = grp % PK_STAGES, qst = grp;   // ring positions of this group's next stage
+        uint32_t uj = (uint32_t)grp, qph = 0;   // its number: use uj / PK_PERIOD of the (position, group) barriers
+        while (next_segment(sg)) {
+            const int t_begin = sg.t_begin, t_end = sg.t_end;
+            const uint32_t yoff = (GENERAL && sg.bx != sg.by) ? (uint32_t)TD_PK_BYTES : 0u;   // the columns' block
+            for (int t = t_begin + grp * TD_ST; t < t_begin + sg.ngroups * TD_GROUP; t += 2 * TD_ST) {
                 const int rows_valid = t_end - t;  // <= 0 in a padding stage: all-zero operands
-                ptx::mbar_wait(pk_full(pst), pph);
-                const uint32_t src = pk0 + pst * TD_PK_BYTES;
+                ptx::mbar_wait(pk_full(pst, grp), (uj / PK_PERIOD) & 1u);
+                const uint32_t src = pk0 + pst * PK_BYTES;
                 // ---- loads first: four transposing loads (rows' planes), four 16-byte chunks (columns' planes)
                 uint32_t xa[2][4], xb[2][4];
 #pragma unroll
@@ -233,7 +262,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
                 uint4 wy[4];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) wy[c] = *reinterpret_cast<const uint4 *>(gbase + (src - base) + 2048 * c + gt * 16);
+                for (int c = 0; c < 4; ++c) wy[c] = *reinterpret_cast<const uint4 *>(gbase + (src + yoff - base) + 2048 * c + gt * 16);
                 ptx::mbar_wait(pl_empty(qst), qph ^ 1u);
                 // ---- A planes -> TMEM
 #pragma unroll
@@ -278,10 +307,11 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 __syncwarp();
                 if (lane == 0) {
                     ptx::mbar_arrive(pl_full(qst));
-                    ptx::mbar_arrive(pk_empty(pst));
+                    ptx::mbar_arrive(pk_empty(pst, grp));
                 }
+                uj += 2;
                 pst += 2;
-                if (pst >= TD_PK_STAGES) { pst -= TD_PK_STAGES; pph ^= 1u; }
+                if (pst >= PK_STAGES) pst -= PK_STAGES;
                 qst += 2;
                 if (qst >= TD_PL_STAGES) { qst -= TD_PL_STAGES; qph ^= 1u; }
             }
@@ -300,35 +330,59 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const int r = 32 * q + lane;                       // row of the tile
         const int sub = p.sub;                             // 128, or 64: two channels per tile
         const int cs = (sub == 64) ? (r >> 6) : 0;         // channel of the tile this row belongs to
-        const int xl = r - cs * sub;                       // input index inside its channel
+        const int xl0 = r - cs * sub;                      // input index inside its channel (block 0)
         const int cpt = 128 / sub;
-        const int img0 = (r < 64) ? 0 : 64;                // tile column held by slot `par` of this row's image
-        const uint32_t srow = epi0 + (r < 64 ? (uint32_t)r * TD_PITCH_LO : 64u * TD_PITCH_LO + (uint32_t)(r - 64) * TD_PITCH_HI);
+        // image of this row.  One block per channel (!GENERAL): rows 0..63 hold 128 columns, rows 64..127 columns 64..127,
+        // all at once.  GENERAL: the image has 64 rows of 128 columns; rows 0..63 of the block use it first, rows 64..127
+        // once those have left (named barrier 2), and the next block's rows 0..63 once these have (named barrier 3)
+        const uint32_t srow = GENERAL ? epi0 + (uint32_t)(r & 63) * TD_PITCH_LO
+                                      : epi0 + (r < 64 ? (uint32_t)r * TD_PITCH_LO : 64u * TD_PITCH_LO + (uint32_t)(r - 64) * TD_PITCH_HI);
         uint8_t *srow_g = epi_g + (srow - epi0);
         const long long Bn = (long long)p.n_out * ((long long)p.n_out + 1) / 2;
         const bool add = (p.out_mode != OUT_STORE);
         const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
         uint32_t acc_ph = 0;
-        for (;;) {
-            int f, t_begin, t_end, ngroups;
-            if (!next_segment(f, t_begin, t_end, ngroups)) break;
+        bool first_segment = true;
+        while (next_segment(sg)) {
+            const bool diag = !GENERAL || sg.bx == sg.by;
+            const int x0 = sg.bx * 128, y0 = sg.by * 128;   // first input of the rows / columns (0 unless GENERAL)
+            const int xl = xl0 + x0;
+            const int img0 = (!GENERAL && r >= 64) ? 64 : 0;   // tile column held by slot `par` of this row's image
             // 8-byte index in vis of (this row, tile column img0) -- formal when that column is left of the diagonal:
             // only its parity and offsets from it are used
-            const long long gi0 = (long long)(f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +
-                                  (img0 - cs * sub);
+            const long long gi0 = (long long)(sg.f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +
+                                  (y0 + img0 - cs * sub);
             int2 *gimg = reinterpret_cast<int2 *>(p.vis) + gi0;
             const uint32_t par = (uint32_t)(reinterpret_cast<uintptr_t>(gimg) >> 3) & 1u;
             ptx::bulk_wait_read0();  // this thread's previous row segment has left shared memory
+            if (GENERAL) {
+                // rows 64..127 of the previous block have left the image (every thread has waited for its own copies)
+                if (!first_segment) ptx::named_bar_sync(3, 32 * TD_EPI_WARPS);
+                first_segment = false;
+            }
             ptx::mbar_wait(acc_full, acc_ph);
             acc_ph ^= 1u;
             ptx::tc_fence_after_sync();
+            // columns this thread sends: [jlo, jhi) of the tile
+            int jlo, jhi;
+            if (diag) {
+                jlo = max(64 * h, r);
+                jhi = min(64 * h + 64, cs * sub + p.n_out - x0);
+                if (sub == 64 && h != cs) jhi = jlo;
+            } else {
+                jlo = 64 * h;
+                jhi = min(64 * h + 64, p.n_out - y0);
+            }
+            const bool row_ok = xl < p.n_out;
+            if (GENERAL && q >= 2) ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);   // rows 0..63 have left the image
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int col = 64 * h + 16 * c;
                 // warp-uniform: the chunk is left of the diagonal for every row of the warp, outside the matrix, or
                 // (two channels per tile) in the other channel's columns
-                const bool skip = (col + 15 < 32 * q) ||
-                                  (sub == 128 ? (col >= p.n_out || 32 * q >= p.n_out) : ((col >> 6) != (q >> 1)));
+                bool skip;
+                if (diag) skip = (col + 15 < 32 * q) || (sub == 128 ? (x0 + col >= p.n_out || x0 + 32 * q >= p.n_out) : ((col >> 6) != (q >> 1)));
+                else skip = (y0 + col >= p.n_out) || (x0 + 32 * q >= p.n_out);
                 if (!skip) {
                     uint32_t ir[16], rr[16], ri[16];
                     ptx::tmem_ld16(trow + col, ir);
@@ -348,10 +402,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             ptx::tc_fence_before_sync();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(acc_empty);
-            // ---- the row segment [jlo, jhi) of tile columns this thread sends
-            int jlo = max(64 * h, r), jhi = min(64 * h + 64, cs * sub + p.n_out);
-            if (sub == 64 && h != cs) jhi = jlo;
-            if (xl < p.n_out && jlo < jhi) {
+            if (row_ok && jlo < jhi) {
                 ptx::fence_proxy_async_smem();  // this thread's st.shared -> visible to the bulk-copy engine
                 int a = jlo - img0, b = jhi - img0;   // as offsets from the image's first column
                 if ((par + a) & 1) {             // leading baseline on an odd 8-byte slot
@@ -372,6 +423,10 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
             }
             ptx::bulk_commit();
+            if (GENERAL && q < 2) {              // rows 64..127 may have the image once these rows have been read
+                ptx::bulk_wait_read0();
+                ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);
+            }
         }
         ptx::bulk_wait0();  // every row segment has been written before the CTA retires
     }

@@ -225,6 +225,27 @@ def test_diagonal_block_kernel(corr, oracle, shape, shares, monkeypatch):
             assert np.array_equal(got, oracle.level1(packed)), (shape, hex(byte))
 
 
+@pytest.mark.parametrize("shares", ["0", "1"])
+@pytest.mark.parametrize("shape", [(256, 3, 20000), (256, 40, 300), (272, 3, 777), (400, 1, 300), (512, 2, 257), (130, 5, 64),
+                                   (200, 2, 5000), (192, 1, 1)])
+def test_diagonal_block_kernel_with_off_diagonal_blocks(corr, oracle, shape, shares, monkeypatch):
+    # corr_tcd_kernel<true>: several 128-blocks per channel (automatic for 128 < N <= 256 with long segments; here
+    # CORR_TCD_MAX_N lets it take every shape): off-diagonal blocks load two packed blocks per stage and write all
+    # 128 x 128 baselines, the row image is used by the two halves of a block in turn.  Ragged N (also N % 16 != 0) and T,
+    # both schedules, stale output, accumulation
+    monkeypatch.setenv("CORR_TCD_MAX_N", "512")
+    monkeypatch.setenv("CORR_TCD_SHARES", shares)
+    N, F, T = shape
+    packed = workloads.uniform_bytes(N, F, T, seed=N * 5 + F + T)
+    want = oracle.level1(packed)
+    got, info = _run(corr, packed, corr.PATH_TCGEN05, prefill=-559038737)
+    nb = (N + 127) // 128
+    assert info["tiles_per_channel"] == nb * (nb + 1) // 2 and info["tile_x"] == 128
+    assert np.array_equal(got, want), shape
+    again, _ = _run(corr, packed, corr.PATH_TCGEN05, accumulate_into=got.copy())
+    assert np.array_equal(again, 2 * want), (shape, "accumulate")
+
+
 @pytest.mark.parametrize("variant", ["1", "3", "5"])
 def test_every_tcgen05_kernel_variant(corr, oracle, variant, monkeypatch):
     # CORR_TC_VARIANT forces the kernel at plan creation: 1 single-CTA tiles with both operands in shared memory (round 1's kernel; N <= 128 runs corr_tcd_kernel unless this forces it), 3 CTA pair
