@@ -1,5 +1,6 @@
-// corr_tcd.cuh -- steps S1-S5 for N <= 128: one 128 x 128 tile per channel, the DIAGONAL block, on one CTA, with the
-// A operand in tensor memory.
+// corr_tcd.cuh -- steps S1-S5 for N <= 256: 128 x 128 tiles, one CTA each, with the A operand in tensor memory.
+// corr_tcd_kernel<false>: one tile per channel, the DIAGONAL block (N <= 128, and two channels of 64 inputs per tile);
+// corr_tcd_kernel<true>: every block of the triangle (128 < N <= 256 by default), see the template's comment.
 //
 // Same mathematics as the other tcgen05 kernels (Eq. 1, summed over time PAPER.md:48, upper triangle
 // PAPER.md:50; x16 int8 operand planes, results shifted right by 8 in the epilogue).  corr_tc.cuh serves these sizes
