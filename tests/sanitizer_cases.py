@@ -26,11 +26,14 @@ import paper_1503_06203_b200 as corr
 import workloads
 
 
-def run(name, packed, path, variant=None, accumulate=False):
+def run(name, packed, path, variant=None, accumulate=False, env=None):
     if variant:
         os.environ["CORR_TC_VARIANT"] = variant
     else:
         os.environ.pop("CORR_TC_VARIANT", None)
+    for k in ("CORR_TCD_MAX_N", "CORR_TCD_SHARES"):
+        os.environ.pop(k, None)
+    os.environ.update(env or {})
     T, F, N = packed.shape
     want = oracle.level1(packed)
     with corr.Plan(N, F, T, path) as plan:
@@ -68,6 +71,19 @@ def cases(s0):
     ok &= run("tc5 transposed tiles, ragged N and T", workloads.uniform_bytes(400, 2, 777, seed=s0 + 5), corr.PATH_TCGEN05, "5")
     # corr_tcd_kernel: one CTA per channel's block (N <= 128), padded stream
     ok &= run("tcd one block per channel", workloads.uniform_bytes(100, 3, 3000, seed=s0 + 6), corr.PATH_TCGEN05, None)
+    # ... equal shares (every segment added into a cleared output), two channels of 64 per tile, many segments per CTA
+    ok &= run("tcd equal shares", workloads.uniform_bytes(128, 5, 9000, seed=s0 + 11), corr.PATH_TCGEN05, None,
+              accumulate=True, env={"CORR_TCD_SHARES": "1"})
+    ok &= run("tcd two channels per tile", workloads.uniform_bytes(64, 6, 5000, seed=s0 + 12), corr.PATH_AUTO, None,
+              env={"CORR_TCD_SHARES": "1"})
+    ok &= run("tcd many units per CTA", workloads.uniform_bytes(128, 600, 300, seed=s0 + 13), corr.PATH_TCGEN05, None,
+              env={"CORR_TCD_SHARES": "0"})
+    # corr_tcd_kernel<true>: off-diagonal blocks, the row image handed from one half of a block to the other (named
+    # barriers 2 / 3), (ring position, unpack group) barriers of the double-stage ring
+    ok &= run("tcd off-diagonal blocks, units", workloads.uniform_bytes(256, 70, 700, seed=s0 + 14), corr.PATH_TCGEN05, None,
+              env={"CORR_TCD_MAX_N": "512", "CORR_TCD_SHARES": "0"})
+    ok &= run("tcd off-diagonal blocks, shares", workloads.uniform_bytes(400, 3, 3000, seed=s0 + 15), corr.PATH_TCGEN05, None,
+              accumulate=True, env={"CORR_TCD_MAX_N": "512", "CORR_TCD_SHARES": "1"})
     # corr_imma_kernel: several chunks per strip (shared-memory atomics, global atomics)
     ok &= run("imma several chunks", workloads.uniform_bytes(32, 9, 4099, seed=s0 + 7), corr.PATH_IMMA)
     ok &= run("dp4a", workloads.uniform_bytes(17, 3, 650, seed=s0 + 8), corr.PATH_DP4A)
