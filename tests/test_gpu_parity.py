@@ -494,6 +494,33 @@ def test_no_write_outside_the_output(corr, oracle, case):
             os.environ.pop("CORR_TC_VARIANT", None)
 
 
+@pytest.mark.parametrize("case", [(128, 3, 700, "1"), (100, 2, 520, "0"), (64, 4, 900, "1"), (127, 5, 3000, "1"), (256, 5, 1300, "0"),
+                                  (272, 3, 700, "1"), (250, 2, 9000, "1")])
+def test_no_write_outside_the_output_tcd(corr, oracle, case, monkeypatch):
+    # the same guard words around vis and the input for corr_tcd_kernel: one block per channel, two channels per tile,
+    # several blocks per channel (rows and columns that hang over N), both schedules, store then add
+    import torch
+    N, F, T, shares = case
+    monkeypatch.setenv("CORR_TCD_MAX_N", "512")
+    monkeypatch.setenv("CORR_TCD_SHARES", shares)
+    packed = workloads.uniform_bytes(N, F, T, seed=N * 3 + T)
+    want = oracle.level1(packed)
+    G = 256
+    with corr.Plan(N, F, T, corr.PATH_AUTO if N == 64 else corr.PATH_TCGEN05) as plan:
+        assert plan.info["path"] == corr.PATH_TCGEN05 and plan.info["tile_x"] == 128
+        buf = torch.full((2 * G + plan.vis_elems,), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        vis = buf[G:G + plan.vis_elems].view(F, plan.baselines, 2)
+        inbuf = torch.full((2048 + packed.size,), 0x88, dtype=torch.uint8, device="cuda")
+        dev = inbuf[1024:1024 + packed.size].view(T, F, N)
+        dev.copy_(torch.from_numpy(packed))
+        plan.execute(dev, vis)
+        plan.execute(dev, vis, accumulate=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(vis.cpu().numpy(), 2 * want), case
+        assert (buf[:G] == 0x5A5A5A5A).all() and (buf[G + plan.vis_elems:] == 0x5A5A5A5A).all(), case
+        assert (inbuf[:1024] == 0x88).all() and (inbuf[1024 + packed.size:] == 0x88).all()
+
+
 def test_int8_issue_loop_measurement(corr):
     # measurement aid: a bare tcgen05.mma.kind::i8 issue loop; on a B200 it lands between the power-capped and the
     # boost-clock ceiling (8192 MAC/clk/SM x 148 SMs x 2 ops at 1.3 .. 1.97 GHz)
