@@ -70,7 +70,7 @@ enum {
  *   F  number of frequency channels,       F >= 1
  *   T  time samples per corr_execute call, 1 <= T <= 16 777 215
  * Returns NULL on failure; the reason is in corr_last_error().
- * Automatic choice: N <= 64 -> CORR_PATH_IMMA (except N = 64 with an even F: two channels per tcgen05 tile), larger
+ * Automatic choice: N <= 64 -> CORR_PATH_IMMA (except N = 64 with an even F or F >= 5: two channels per tcgen05 tile), larger
  * N -> CORR_PATH_TCGEN05 (one CTA per 128 x 128 block up to N = 128, and up to N = 256 when T is long enough for
  * segments of 4096 samples; CTA-pair 256 x 128 tiles otherwise).  When
  * N % 16 != 0 these two paths first copy the stream to a plan-owned buffer padded to the next multiple of 16 inputs

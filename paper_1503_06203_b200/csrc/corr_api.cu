@@ -360,9 +360,13 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             // holds two whole channels and its two diagonal 64-blocks are their matrices (half of the tensor work is
             // cross-channel and dropped; still 1.45x the warp-MMA kernel, which is MMA-issue-bound at N = 64,
             // profiles/r02_sweep.md)
-            path = (N == 64 && F % 2 == 0) ? CORR_PATH_TCGEN05 : (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;
+            // (an odd number of channels: the last tile holds one channel and 64 bytes beyond the row, which TMA fills with
+            // zeros; measured against the warp-MMA kernel at T = 65536: F = 3 a tie, F = 5: 19.9 / 26.3 us, F = 63: 82 / 141)
+            path = (N == 64 && (F % 2 == 0 || F >= 5)) ? CORR_PATH_TCGEN05 : (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;
     }
-    const bool packed64 = (path == CORR_PATH_TCGEN05 && N == 64 && F % 2 == 0);
+    const char *v_forced = getenv("CORR_TC_VARIANT");
+    const bool v1_forced = v_forced && !strcmp(v_forced, "1");   // corr_tc_kernel reads the packed view through a 3-D map: even F only
+    const bool packed64 = (path == CORR_PATH_TCGEN05 && N == 64 && (F % 2 == 0 || (F >= 3 && !v1_forced && !(v_forced && v_forced[0]))));
     if (path == CORR_PATH_IMMA && n_pad > 64) {
         g_create_rc = CORR_ERR_UNSUPPORTED; set_err("corr_plan_create: the warp-MMA path takes N <= 64, got N=%d", N);
         return nullptr;
@@ -461,7 +465,7 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (p->variant == 1 && (packed64 || n_pad <= std::max(128, tcd_max)) && !(v && !strcmp(v, "1"))) p->variant = 2;
     }
     p->pack_sub = packed64 ? 64 : 128;
-    const int Ns = packed64 ? 128 : N, Fs = packed64 ? F / 2 : F;   // the shape the tile schedule sees
+    const int Ns = packed64 ? 128 : N, Fs = packed64 ? (F + 1) / 2 : F;   // the shape the tile schedule sees
     const int nb = (Ns + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
     std::vector<ushort4> tiles4;
@@ -696,6 +700,24 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
         p->tmap_ptr = packed_dev;
         return CORR_OK;
     }
+    if (p->pack_sub == 64 && p->variant == 2) {
+        // two channels of 64 inputs per tile (corr_tcd_kernel): the stream as a byte matrix (F * 64, T); tile g is the box
+        // at column 128 g, and with an odd F the last tile's second half lies beyond the row and is filled with zeros
+        const cuuint64_t dims2[2] = {(cuuint64_t)p->F * 64u, (cuuint64_t)p->T};
+        const cuuint64_t strides2[1] = {(cuuint64_t)p->F * 64u};
+        const cuuint32_t box2[2] = {128u, (cuuint32_t)corr::TD_ST};
+        const cuuint32_t estr2[2] = {1u, 1u};
+        CUresult r2 = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(packed_dev), dims2, strides2,
+                                      box2, estr2, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                      p->balanced ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r2 != CUDA_SUCCESS) {
+            set_err("cuTensorMapEncodeTiled (2-D, two channels per tile) failed with CUresult %d (N=%d F=%d T=%d)", (int)r2, p->N, p->F, p->T);
+            return CORR_ERR_CUDA;
+        }
+        p->tmap_ptr = packed_dev;
+        return CORR_OK;
+    }
     // packed[T][F][N] bytes as a 3-D tensor, innermost first: (N, F, T), strides (1, N, F*N) bytes.
     // (two 64-input channels packed into one 128-tile: the same bytes seen as (128, F/2, T))
     const cuuint64_t nw = (p->pack_sub == 64) ? 128 : (cuuint64_t)p->n_pad, fw = (p->pack_sub == 64) ? (cuuint64_t)p->F / 2 : (cuuint64_t)p->F;
@@ -833,7 +855,8 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         } else {
             corr::TcParams prm;
             prm.N = (p->pack_sub == 64) ? 128 : p->N;
-            prm.F = (p->pack_sub == 64) ? p->F / 2 : p->F;
+            prm.F = (p->pack_sub == 64) ? (p->F + 1) / 2 : p->F;
+            prm.f_out = p->F;
             prm.sub = p->pack_sub;
             prm.n_out = p->N;
             prm.T = p->T;

@@ -70,6 +70,7 @@ struct TcParams {
     int sub;           // 128, or 64: the tile holds two whole channels of 64 inputs (N = 128, F = channels / 2); only the
                        // two diagonal 64-blocks are written, as channels 2f and 2f + 1
     int n_out;         // inputs per channel in the layout of vis
+    int f_out;         // corr_tcd_kernel, sub == 64: channels in vis (the last tile holds one channel when this is odd)
     int groups_per_f;  // corr_tcd_kernel, slices == 0: groups of 256 samples per channel, dealt to the CTAs in equal shares
     const ushort2 *tiles;
     int32_t *vis;

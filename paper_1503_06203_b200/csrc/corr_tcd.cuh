@@ -181,7 +181,10 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                         ptx::mbar_wait(pk_empty(st, (int)(jp & 1u)), (jp / PK_PERIOD) & 1u);
                     }
                     ptx::mbar_arrive_expect_tx(pk_full(st, g), (!GENERAL || diag) ? TD_PK_BYTES : 2 * TD_PK_BYTES);
-                    ptx::tma_load_3d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), sg.bx * 128, sg.f, t);
+                    if (!GENERAL && p.sub == 64)   // two channels per tile: the stream as a byte matrix, tile f at column 128 f
+                        ptx::tma_load_2d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), 128 * sg.f, t);
+                    else
+                        ptx::tma_load_3d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), sg.bx * 128, sg.f, t);
                     if (GENERAL && !diag) ptx::tma_load_3d(pk0 + st * PK_BYTES + TD_PK_BYTES, &tmap, pk_full(st, g), sg.by * 128, sg.f, t);
                     ++j;
                     if (++st == PK_STAGES) st = 0;
@@ -374,7 +377,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 jlo = 64 * h;
                 jhi = min(64 * h + 64, p.n_out - y0);
             }
-            const bool row_ok = xl < p.n_out;
+            const bool row_ok = xl < p.n_out && (sub != 64 || sg.f * cpt + cs < p.f_out);
             if (GENERAL && q >= 2) ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);   // rows 0..63 have left the image
 #pragma unroll
             for (int c = 0; c < 4; ++c) {

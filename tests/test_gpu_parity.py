@@ -180,16 +180,17 @@ def test_determinism(corr):
     assert np.array_equal(_run(corr, packed, corr.PATH_IMMA)[0], _run(corr, packed, corr.PATH_TCGEN05)[0])
 
 
-@pytest.mark.parametrize("F", [2, 6, 16, 3])
+@pytest.mark.parametrize("F", [2, 6, 16, 3, 5, 63])
 def test_n64_two_channels_per_tile(corr, oracle, F):
     # N = 64, even F: AUTO runs corr_tcd_kernel (one CTA per 128-block) on the stream seen as [T][F/2][128] and writes the two
-    # diagonal 64-blocks of each tile as channels 2f, 2f + 1; odd F stays on the warp-MMA kernel.  Ragged T, split T,
+    # diagonal 64-blocks of each tile as channels 2f, 2f + 1; an odd F from 5 on as well (the last tile holds one channel
+    # and zeros from beyond the row), a small odd F stays on the warp-MMA kernel.  Ragged T, split T,
     # stale output, accumulation, extreme bytes.
     for T in (1, 63, 300, 4099, 70000 if F == 2 else 1000):
         packed = workloads.uniform_bytes(64, F, T, seed=64 * F + T)
         want = oracle.level1(packed)
         got, info = _run(corr, packed, corr.PATH_AUTO, prefill=-559038737)
-        assert info["path"] == (corr.PATH_TCGEN05 if F % 2 == 0 else corr.PATH_IMMA)
+        assert info["path"] == (corr.PATH_TCGEN05 if (F % 2 == 0 or F >= 5) else corr.PATH_IMMA)
         assert np.array_equal(got, want), (F, T)
         again, _ = _run(corr, packed, corr.PATH_AUTO, accumulate_into=got.copy())
         assert np.array_equal(again, 2 * want), (F, T, "accumulate")
