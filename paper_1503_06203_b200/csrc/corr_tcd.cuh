@@ -81,7 +81,6 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     const uint32_t pl0 = pk0 + PK_STAGES * PK_BYTES;
     const uint32_t epi0 = pl0 + TD_PL_STAGES * TD_PL_BYTES;
     const uint32_t bar0 = epi0 + (GENERAL ? TD_EPI_BYTES_G : TD_EPI_BYTES);
-    uint8_t *epi_g = gbase + (epi0 - base);
     auto pk_full = [&](int s, int g) { return bar0 + 8u * (2 * s + g); };
     auto pk_empty = [&](int s, int g) { return bar0 + 8u * (2 * PK_STAGES + 2 * s + g); };
     auto pl_full = [&](int s) { return bar0 + 8u * (4 * PK_STAGES + s); };
@@ -339,9 +338,8 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // image of this row.  One block per channel (!GENERAL): rows 0..63 hold 128 columns, rows 64..127 columns 64..127,
         // all at once.  GENERAL: the image has 64 rows of 128 columns; rows 0..63 of the block use it first, rows 64..127
         // once those have left (named barrier 2), and the next block's rows 0..63 once these have (named barrier 3)
-        const uint32_t srow = GENERAL ? epi0 + (uint32_t)(r & 63) * TD_PITCH_LO
-                                      : epi0 + (r < 64 ? (uint32_t)r * TD_PITCH_LO : 64u * TD_PITCH_LO + (uint32_t)(r - 64) * TD_PITCH_HI);
-        uint8_t *srow_g = epi_g + (srow - epi0);
+        const uint32_t srow_own = GENERAL ? epi0 + (uint32_t)(r & 63) * TD_PITCH_LO
+                                          : epi0 + (r < 64 ? (uint32_t)r * TD_PITCH_LO : 64u * TD_PITCH_LO + (uint32_t)(r - 64) * TD_PITCH_HI);
         const long long Bn = (long long)p.n_out * ((long long)p.n_out + 1) / 2;
         const bool add = (p.out_mode != OUT_STORE);
         const uint32_t trow = tmem + ((uint32_t)(q * 32) << 16);
@@ -352,6 +350,12 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int x0 = sg.bx * 128, y0 = sg.by * 128;   // first input of the rows / columns (0 unless GENERAL)
             const int xl = xl0 + x0;
             const int img0 = (!GENERAL && r >= 64) ? 64 : 0;   // tile column held by slot `par` of this row's image
+            // GENERAL, the CTA's last segment: nothing is loaded any more, so rows 64..127 take the packed ring as their
+            // image instead of waiting for rows 0..63 to leave theirs
+            const bool last = GENERAL && it >= it_end;
+            static_assert(TD_EPI_BYTES_G <= TD_PK_STAGES_G * 2 * TD_PK_BYTES, "the packed ring holds an image");
+            const uint32_t srow = (last && q >= 2) ? pk0 + (uint32_t)(r & 63) * TD_PITCH_LO : srow_own;
+            uint8_t *srow_g = gbase + (srow - base);
             // 8-byte index in vis of (this row, tile column img0) -- formal when that column is left of the diagonal:
             // only its parity and offsets from it are used
             const long long gi0 = (long long)(sg.f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +
@@ -378,7 +382,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 jhi = min(64 * h + 64, p.n_out - y0);
             }
             const bool row_ok = xl < p.n_out && (sub != 64 || sg.f * cpt + cs < p.f_out);
-            if (GENERAL && q >= 2) ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);   // rows 0..63 have left the image
+            if (GENERAL && !last && q >= 2) ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);   // rows 0..63 have left the image
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const int col = 64 * h + 16 * c;
@@ -427,7 +431,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
             }
             ptx::bulk_commit();
-            if (GENERAL && q < 2) {              // rows 64..127 may have the image once these rows have been read
+            if (GENERAL && !last && q < 2) {     // rows 64..127 may have the image once these rows have been read
                 ptx::bulk_wait_read0();
                 ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);
             }
