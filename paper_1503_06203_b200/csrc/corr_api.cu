@@ -174,6 +174,9 @@ struct corr_plan {
                        // for N <= 128, where a pair tile would be half empty, and for two 64-input channels per tile);
                        // 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default above N = 128);
                        // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
+    int win_ok;        // variant 2, N % 16 != 0: the unpadded stream can be read through 16-byte aligned windows (corr_tcd.cuh):
+                       // N + 15 <= 128 and (F * N) % 16 == 0; used when the caller's buffer is 16-byte aligned, else the padded copy
+    int tmap_win;      // the cached tensor map is the window one
     int balanced;      // variant 2: all groups of all channels dealt to the CTAs in equal shares (corr_tcd.cuh), output added
     int groups_full, groups_last;   // variant 3: groups of T3_GROUP samples per full / last slice
     long long total_groups;
@@ -531,7 +534,8 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (e && G >= 1) p->balanced = (e[0] != '0') ? 1 : 0;
         if (p->balanced) p->grid = (int)std::min<long long>(G, p->sm_count);
     }
-    p->kernels_per_exec = 1 + ((path != CORR_PATH_DP4A && n_pad != N) ? 1 : 0);  // + corr_pad_kernel
+    p->win_ok = (p->variant == 2 && !packed64 && n_pad != N && N + 15 <= 128 && ((long long)F * N) % 16 == 0 && !getenv("CORR_TCD_NO_WINDOW")) ? 1 : 0;
+    p->kernels_per_exec = 1 + ((path != CORR_PATH_DP4A && n_pad != N && !p->win_ok) ? 1 : 0);  // + corr_pad_kernel (with win_ok: only for a misaligned buffer)
     p->aligned = (N % 4 == 0) ? 1 : 0;
     if (p->variant >= 3) {
         p->groups_full = p->t_per_slice / corr::T3_GROUP;
@@ -681,9 +685,10 @@ int corr_time_shift(int N, int F, int T, const uint8_t *packed_in_dev, const int
     return CORR_OK;
 }
 
-static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
+static int build_tmap(corr_plan *p, const uint8_t *packed_dev, int window = 0)
 {
-    if (p->tmap_ptr == packed_dev) return CORR_OK;
+    if (p->tmap_ptr == packed_dev && p->tmap_win == window) return CORR_OK;
+    p->tmap_win = window;
     if (p->path == CORR_PATH_IMMA) {
         // packed[T][F][N] as a byte matrix, innermost first: (F*N, T), row stride F*N bytes
         const cuuint64_t dims2[2] = {(cuuint64_t)p->F * (cuuint64_t)p->n_pad, (cuuint64_t)p->T};
@@ -695,6 +700,23 @@ static int build_tmap(corr_plan *p, const uint8_t *packed_dev)
                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r2 != CUDA_SUCCESS) {
             set_err("cuTensorMapEncodeTiled (2-D) failed with CUresult %d (N=%d F=%d T=%d)", (int)r2, p->N, p->F, p->T);
+            return CORR_ERR_CUDA;
+        }
+        p->tmap_ptr = packed_dev;
+        return CORR_OK;
+    }
+    if (window) {
+        // the unpadded stream as a byte matrix (F * N, T): channel f is read through the box at column f * N rounded down to 16
+        const cuuint64_t dims2[2] = {(cuuint64_t)p->F * (cuuint64_t)p->N, (cuuint64_t)p->T};
+        const cuuint64_t strides2[1] = {(cuuint64_t)p->F * (cuuint64_t)p->N};
+        const cuuint32_t box2[2] = {128u, (cuuint32_t)corr::TD_ST};
+        const cuuint32_t estr2[2] = {1u, 1u};
+        CUresult r2 = get_encode_fn()(&p->tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(packed_dev), dims2, strides2,
+                                      box2, estr2, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                      p->balanced ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r2 != CUDA_SUCCESS) {
+            set_err("cuTensorMapEncodeTiled (2-D, windows) failed with CUresult %d (N=%d F=%d T=%d)", (int)r2, p->N, p->F, p->T);
             return CORR_ERR_CUDA;
         }
         p->tmap_ptr = packed_dev;
@@ -762,7 +784,9 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         return CORR_ERR_INVALID_ARG;
     }
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    if (padded) {
+    // N % 16 != 0, N <= 113, rows of a multiple of 16 bytes, an aligned buffer: corr_tcd_kernel reads the stream as it is
+    const int window = (padded && p->variant == 2 && p->win_ok && !(reinterpret_cast<uintptr_t>(packed_dev) & 15u)) ? 1 : 0;
+    if (padded && !window) {
         // N % 16 != 0: the TMA-fed kernels read a copy of the stream padded to n_pad inputs with stored zeros
         const long long rows = (long long)p->T * p->F;
         corr::corr_pad_kernel<<<8 * p->sm_count, 256, 0, stream>>>(packed_dev, p->pad_buf, p->N, p->n_pad, rows);
@@ -814,7 +838,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             break;
         }
     } else {
-        int rc = build_tmap(p, packed_dev);
+        int rc = build_tmap(p, packed_dev, window);
         if (rc != CORR_OK) return rc;
         if (p->variant >= 3) {
             corr::Tc3Params prm;
@@ -857,6 +881,7 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
             prm.N = (p->pack_sub == 64) ? 128 : p->N;
             prm.F = (p->pack_sub == 64) ? (p->F + 1) / 2 : p->F;
             prm.f_out = p->F;
+            prm.win_n = window ? p->N : 0;
             prm.sub = p->pack_sub;
             prm.n_out = p->N;
             prm.T = p->T;

@@ -70,6 +70,9 @@ struct TcParams {
     int sub;           // 128, or 64: the tile holds two whole channels of 64 inputs (N = 128, F = channels / 2); only the
                        // two diagonal 64-blocks are written, as channels 2f and 2f + 1
     int n_out;         // inputs per channel in the layout of vis
+    int win_n;         // corr_tcd_kernel<false>, > 0: the unpadded stream of win_n inputs per channel (win_n % 16 != 0) read through
+                       // windows of 128 bytes that start on 16-byte boundaries; channel f is rows / columns o .. o + win_n - 1 of
+                       // its tile, o = (f * win_n) % 16
     int f_out;         // corr_tcd_kernel, sub == 64: channels in vis (the last tile holds one channel when this is odd)
     int groups_per_f;  // corr_tcd_kernel, slices == 0: groups of 256 samples per channel, dealt to the CTAs in equal shares
     const ushort2 *tiles;

@@ -226,6 +226,35 @@ def test_diagonal_block_kernel(corr, oracle, shape, shares, monkeypatch):
             assert np.array_equal(got, oracle.level1(packed)), (shape, hex(byte))
 
 
+@pytest.mark.parametrize("shape", [(100, 64, 3000), (100, 4, 777), (113, 16, 1000), (65, 16, 20000), (72, 2, 300), (97, 32, 257),
+                                   (104, 6, 5000)])
+def test_unpadded_stream_through_aligned_windows(corr, oracle, shape, monkeypatch):
+    # N % 16 != 0, N <= 113 and rows of a multiple of 16 bytes: corr_tcd_kernel reads the stream as it is, channel f through
+    # the 128-byte window at column f N rounded down to 16 (its inputs are rows / columns (f N) % 16 ... of the tile; what the
+    # window holds of the neighbouring channels is computed and dropped).  Both schedules; a buffer that is not 16-byte
+    # aligned takes the padded copy instead; same bits either way
+    import torch
+    N, F, T = shape
+    packed = workloads.uniform_bytes(N, F, T, seed=N + F + T)
+    want = oracle.level1(packed)
+    for shares in ("0", "1"):
+        monkeypatch.setenv("CORR_TCD_SHARES", shares)
+        for off in (0, 3):
+            with corr.Plan(N, F, T, corr.PATH_TCGEN05) as plan:
+                assert plan.info["kernels"] == 1
+                raw = torch.full((packed.size + 64,), 0x88, dtype=torch.uint8, device="cuda")
+                dev = raw[off:off + packed.size].view(T, F, N)
+                dev.copy_(torch.from_numpy(packed))
+                vis = plan.new_vis()
+                vis.fill_(-559038737)
+                plan.execute(dev, vis)
+                torch.cuda.synchronize()
+                assert np.array_equal(vis.cpu().numpy(), want), (shape, shares, off)
+                plan.execute(dev, vis, accumulate=True)
+                torch.cuda.synchronize()
+                assert np.array_equal(vis.cpu().numpy(), 2 * want), (shape, shares, off, "accumulate")
+
+
 @pytest.mark.parametrize("shares", ["0", "1"])
 @pytest.mark.parametrize("shape", [(256, 3, 20000), (256, 40, 300), (272, 3, 777), (400, 1, 300), (512, 2, 257), (130, 5, 64),
                                    (200, 2, 5000), (192, 1, 1)])
