@@ -41,7 +41,7 @@ constexpr int IM_ROWS = 128;                 // time samples per stage
 constexpr int IM_STAGE_BYTES = IM_ROWS * 128;
 constexpr int IM_STAGES = 6;
 constexpr int IM_MAX_CHUNK = 32768;          // time samples per CTA: 256 * 128 * chunk stays far below 2^31 (multiple of IM_ROWS)
-constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 256;
+constexpr int IM_SMEM_BYTES = 1024 + IM_STAGES * IM_STAGE_BYTES + 512;   // ring + 2 x IM_STAGES x 4 barriers
 
 template <int NT16> struct ImmaCfg {
     static constexpr int N = 16 * NT16;
@@ -96,8 +96,16 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t *gbase = smem_raw + (base - ptx::smem_u32(smem_raw));
     const uint32_t bar0 = base + IM_STAGES * IM_STAGE_BYTES;
-    auto full = [&](int s) { return bar0 + 8u * s; };
-    auto empty = [&](int s) { return bar0 + 8u * (IM_STAGES + s); };
+    // One pair of barriers per (ring position, K-split group).  Stage j goes to position j % IM_STAGES and is consumed by the
+    // warps of group j % KS only, so with IM_STAGES = 6 and KS = 4 a group comes back to a position every SECOND time round:
+    // on a barrier per position it would always wait for the same parity and could not tell "my stage has landed" from
+    // "the other group's stage before it has not landed yet" (TMA loads complete out of order): it would read the ring
+    // early and arrive on `empty` once too often.  With a barrier of its own every visit is the next phase; a (position,
+    // group) pair is used once every PERIOD = lcm(IM_STAGES, KS) stages.
+    constexpr int PERIOD = (IM_STAGES % C::KS == 0) ? IM_STAGES : (IM_STAGES * C::KS) / ((IM_STAGES % 2 == 0 && C::KS % 2 == 0) ? 2 : 1);
+    static_assert(PERIOD % IM_STAGES == 0 && PERIOD % C::KS == 0 && C::KS <= 4, "PERIOD = lcm(IM_STAGES, KS)");
+    auto full = [&](int s, int g) { return bar0 + 8u * (4 * s + g); };
+    auto empty = [&](int s, int g) { return bar0 + 8u * (4 * IM_STAGES + 4 * s + g); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int strip = blockIdx.x, chunk = blockIdx.y;
@@ -108,8 +116,10 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     if (threadIdx.x == 0) {
         ptx::prefetch_tmap(&tmap);
         for (int s = 0; s < IM_STAGES; ++s) {
-            ptx::mbar_init(full(s), 1);
-            ptx::mbar_init(empty(s), C::WARPS / C::KS);   // the warps that own the stage (see the K-split below)
+            for (int g = 0; g < C::KS; ++g) {
+                ptx::mbar_init(full(s, g), 1);
+                ptx::mbar_init(empty(s, g), C::WARPS / C::KS);   // the warps of the group (see the K-split below)
+            }
         }
         ptx::fence_mbar_init();
     }
@@ -133,9 +143,12 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
     auto produce = [&](int j) {
         if (j < nstages) {
             const int sj = j % IM_STAGES;
-            ptx::mbar_wait(empty(sj), ((uint32_t)(j / IM_STAGES) & 1u) ^ 1u);
-            ptx::mbar_arrive_expect_tx(full(sj), IM_STAGE_BYTES);
-            ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj), strip * C::STRIP, t_begin + j * IM_ROWS);
+            if (j >= IM_STAGES) {   // the position's last stage, j - IM_STAGES (another group's when KS = 4), has been consumed
+                const int jp = j - IM_STAGES;
+                ptx::mbar_wait(empty(sj, jp % C::KS), (uint32_t)(jp / PERIOD) & 1u);
+            }
+            ptx::mbar_arrive_expect_tx(full(sj, j % C::KS), IM_STAGE_BYTES);
+            ptx::tma_load_2d(base + sj * IM_STAGE_BYTES, &tmap, full(sj, j % C::KS), strip * C::STRIP, t_begin + j * IM_ROWS);
         }
     };
     if (warp == C::WARPS) {
@@ -150,7 +163,7 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
         // load / unpack phase of one overlaps the MMA phase of another instead of all four moving in lockstep.
         for (int it = ks; it < nstages; it += C::KS) {
             const int s = it % IM_STAGES;
-            ptx::mbar_wait(full(s), (uint32_t)(it / IM_STAGES) & 1u);
+            ptx::mbar_wait(full(s, ks), (uint32_t)(it / PERIOD) & 1u);
             const uint32_t stage = base + s * IM_STAGE_BYTES;
             if (f < p.F) {
 #pragma unroll
@@ -195,7 +208,7 @@ corr_imma_kernel(const __grid_constant__ CUtensorMap tmap, const ImmaParams p)
                 }
             }
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty(s));
+            if (lane == 0) ptx::mbar_arrive(empty(s, ks));
         }
     }
 
