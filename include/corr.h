@@ -74,8 +74,9 @@ enum {
  * N -> CORR_PATH_TCGEN05 (one CTA per 128 x 128 block up to N = 128, and up to N = 256 when T is long enough for
  * segments of 4096 samples; CTA-pair 256 x 128 tiles otherwise).  When
  * N % 16 != 0 these two paths first copy the stream to a plan-owned buffer padded to the next multiple of 16 inputs
- * (TMA strides and box start addresses are multiples of 16 bytes) -- except 64 < N <= 113 with F*N % 16 == 0 and a
- * 16-byte aligned packed_dev, which the tcgen05 path reads in place through 16-byte aligned windows; CORR_PATH_DP4A takes any N without a copy and is
+ * (TMA strides and box start addresses are multiples of 16 bytes) -- except N <= 113 with F*N % 16 == 0 and a
+ * 16-byte aligned packed_dev, which the tcgen05 path reads in place through 16-byte aligned windows (the automatic
+ * choice for such N below 64 as well; there a misaligned packed_dev is CORR_ERR_INVALID_ARG); CORR_PATH_DP4A takes any N without a copy and is
  * only used on request.  Testing aids (environment, read at plan creation): CORR_FORCE_PATH=dp4a|tcgen05|imma
  * overrides the choice; CORR_TC_VARIANT=1|3|5 forces the tcgen05 kernel (1 single-CTA tiles with both operands in
  * shared memory -- the round-1 kernel the N <= 128 kernel replaced --, 3 CTA pairs, 5 = CTA

@@ -174,6 +174,7 @@ struct corr_plan {
                        // for N <= 128, where a pair tile would be half empty, and for two 64-input channels per tile);
                        // 3: CTA-pair tiles 256x128, A operand in TMEM (corr_tc3.cuh, default above N = 128);
                        // 5: as 3 with three products per complex MAC (corr_tc5.cuh; CORR_TC_VARIANT=5)
+    int win_c, Fs;     // whole channels per window ((128 - 15) / N; > 1: the buffer MUST be aligned); channels as the schedule sees them
     int win_ok;        // variant 2, N % 16 != 0: the unpadded stream can be read through 16-byte aligned windows (corr_tcd.cuh):
                        // N + 15 <= 128 and (F * N) % 16 == 0; used when the caller's buffer is 16-byte aligned, else the padded copy
     int tmap_win;      // the cached tensor map is the window one
@@ -210,7 +211,7 @@ extern "C" void corr_plan_destroy(corr_plan *p);
 // corr_execute only enqueues work (no allocation, no implicit synchronisation, capturable into a CUDA graph).
 static bool alloc_pad_buf(corr_plan *p)
 {
-    if (p->path == CORR_PATH_DP4A || p->n_pad == p->N) return true;
+    if (p->path == CORR_PATH_DP4A || p->n_pad == p->N || p->win_c > 1) return true;   // (win_c > 1: never padded)
     if (cudaMalloc(&p->pad_buf, (size_t)p->T * p->F * p->n_pad) != cudaSuccess) {
         g_create_rc = CORR_ERR_ALLOC;
         set_err("corr_plan_create: device allocation of the padded stream (%zu bytes) failed: %s",
@@ -366,6 +367,9 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
             // (an odd number of channels: the last tile holds one channel and 64 bytes beyond the row, which TMA fills with
             // zeros; measured against the warp-MMA kernel at T = 65536: F = 3 a tie, F = 5: 19.9 / 26.3 us, F = 63: 82 / 141)
             path = (N == 64 && (F % 2 == 0 || F >= 5)) ? CORR_PATH_TCGEN05 : (n_pad <= 64) ? CORR_PATH_IMMA : CORR_PATH_TCGEN05;
+            // N % 16 != 0 below 64 with rows of a multiple of 16 bytes: several whole channels per 16-byte aligned window of
+            // corr_tcd_kernel instead of a padded copy + the warp-MMA kernel (N = 37, F = 128, T = 32768: 68 against 224 us)
+            if (path == CORR_PATH_IMMA && n_pad != N && ((long long)F * N) % 16 == 0 && !getenv("CORR_TCD_NO_WINDOW")) path = CORR_PATH_TCGEN05;
     }
     const char *v_forced = getenv("CORR_TC_VARIANT");
     const bool v1_forced = v_forced && !strcmp(v_forced, "1");   // corr_tc_kernel reads the packed view through a 3-D map: even F only
@@ -468,7 +472,15 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (p->variant == 1 && (packed64 || n_pad <= std::max(128, tcd_max)) && !(v && !strcmp(v, "1"))) p->variant = 2;
     }
     p->pack_sub = packed64 ? 64 : 128;
-    const int Ns = packed64 ? 128 : N, Fs = packed64 ? (F + 1) / 2 : F;   // the shape the tile schedule sees
+    // N % 16 != 0 read through 16-byte aligned windows (corr_tcd.cuh): N <= 113, rows of a multiple of 16 bytes; a window holds
+    // (128 - 15) / N whole channels
+    int win_c = 0;
+    if (p->variant == 2 && !packed64 && n_pad != N && N + 15 <= 128 && ((long long)F * N) % 16 == 0 && !getenv("CORR_TCD_NO_WINDOW"))
+        win_c = (128 - 15) / N;
+    p->win_c = win_c;
+    p->win_ok = win_c > 0 ? 1 : 0;
+    const int Ns = packed64 ? 128 : N, Fs = packed64 ? (F + 1) / 2 : (win_c > 1) ? (F + win_c - 1) / win_c : F;   // the shape the tile schedule sees
+    p->Fs = Fs;
     const int nb = (Ns + p->tile - 1) / p->tile;
     std::vector<ushort2> tiles;
     std::vector<ushort4> tiles4;
@@ -534,7 +546,6 @@ corr_plan *corr_plan_create_ex(int N, int F, int T, int path)
         if (e && G >= 1) p->balanced = (e[0] != '0') ? 1 : 0;
         if (p->balanced) p->grid = (int)std::min<long long>(G, p->sm_count);
     }
-    p->win_ok = (p->variant == 2 && !packed64 && n_pad != N && N + 15 <= 128 && ((long long)F * N) % 16 == 0 && !getenv("CORR_TCD_NO_WINDOW")) ? 1 : 0;
     p->kernels_per_exec = 1 + ((path != CORR_PATH_DP4A && n_pad != N && !p->win_ok) ? 1 : 0);  // + corr_pad_kernel (with win_ok: only for a misaligned buffer)
     p->aligned = (N % 4 == 0) ? 1 : 0;
     if (p->variant >= 3) {
@@ -786,6 +797,10 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     // N % 16 != 0, N <= 113, rows of a multiple of 16 bytes, an aligned buffer: corr_tcd_kernel reads the stream as it is
     const int window = (padded && p->variant == 2 && p->win_ok && !(reinterpret_cast<uintptr_t>(packed_dev) & 15u)) ? 1 : 0;
+    if (padded && p->variant == 2 && p->win_c > 1 && !window) {
+        set_err("corr_execute: packed_dev must be 16-byte aligned for this shape (N=%d: %d channels per 128-byte window)", p->N, p->win_c);
+        return CORR_ERR_INVALID_ARG;
+    }
     if (padded && !window) {
         // N % 16 != 0: the TMA-fed kernels read a copy of the stream padded to n_pad inputs with stored zeros
         const long long rows = (long long)p->T * p->F;
@@ -879,9 +894,10 @@ int corr_execute(corr_plan *p, const uint8_t *packed_dev, int32_t *vis_dev, int 
         } else {
             corr::TcParams prm;
             prm.N = (p->pack_sub == 64) ? 128 : p->N;
-            prm.F = (p->pack_sub == 64) ? (p->F + 1) / 2 : p->F;
+            prm.F = p->Fs;
             prm.f_out = p->F;
             prm.win_n = window ? p->N : 0;
+            prm.win_c = p->win_c;
             prm.sub = p->pack_sub;
             prm.n_out = p->N;
             prm.T = p->T;

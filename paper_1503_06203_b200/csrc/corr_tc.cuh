@@ -73,7 +73,8 @@ struct TcParams {
     int win_n;         // corr_tcd_kernel<false>, > 0: the unpadded stream of win_n inputs per channel (win_n % 16 != 0) read through
                        // windows of 128 bytes that start on 16-byte boundaries; channel f is rows / columns o .. o + win_n - 1 of
                        // its tile, o = (f * win_n) % 16
-    int f_out;         // corr_tcd_kernel, sub == 64: channels in vis (the last tile holds one channel when this is odd)
+    int win_c;         // ... whole channels per window ((128 - 15) / win_n): tile g holds channels g win_c .. g win_c + win_c - 1
+    int f_out;         // corr_tcd_kernel, sub == 64 or windows: channels in vis (the last tile holds one channel when this is odd)
     int groups_per_f;  // corr_tcd_kernel, slices == 0: groups of 256 samples per channel, dealt to the CTAs in equal shares
     const ushort2 *tiles;
     int32_t *vis;

@@ -181,7 +181,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     }
                     ptx::mbar_arrive_expect_tx(pk_full(st, g), (!GENERAL || diag) ? TD_PK_BYTES : 2 * TD_PK_BYTES);
                     if (!GENERAL && p.win_n > 0)   // unpadded stream: the window of channel f starts at column f * N rounded down to 16
-                        ptx::tma_load_2d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), (sg.f * p.win_n) & ~15, t);
+                        ptx::tma_load_2d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), (sg.f * p.win_c * p.win_n) & ~15, t);
                     else if (!GENERAL && p.sub == 64)   // two channels per tile: the stream as a byte matrix, tile f at column 128 f
                         ptx::tma_load_2d(pk0 + st * PK_BYTES, &tmap, pk_full(st, g), 128 * sg.f, t);
                     else
@@ -352,8 +352,19 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int x0 = sg.bx * 128, y0 = sg.by * 128;   // first input of the rows / columns (0 unless GENERAL)
             // window mode: the channel's inputs are rows / columns wo .. wo + N - 1 of the tile (the bytes before belong to
             // the previous channel, the bytes after to the next: computed and dropped)
-            const int wo = (!GENERAL && p.win_n > 0) ? ((sg.f * p.win_n) & 15) : 0;
-            const int xl = xl0 + x0 - wo;
+            // ... and with several whole channels per window (win_c > 1, small N) the row's channel is the k-th of the tile
+            int xl = xl0 + x0, chan = sg.f * cpt + cs, coff = cs * sub, cend = p.n_out;
+            bool win_valid = true;
+            if (!GENERAL && p.win_n > 0) {
+                const int wo = (sg.f * p.win_c * p.win_n) & 15;
+                const int rel = r - wo;
+                const int wk = rel >= 0 ? rel / p.win_n : 0;
+                xl = rel - wk * p.win_n;
+                chan = sg.f * p.win_c + wk;
+                coff = wo + wk * p.win_n;          // tile column of the channel's input 0
+                cend = wo + p.win_c * p.win_n;     // end of the tile's last channel
+                win_valid = rel >= 0 && wk < p.win_c && chan < p.f_out;
+            }
             const int img0 = (!GENERAL && r >= 64) ? 64 : 0;   // tile column held by slot `par` of this row's image
             // GENERAL, the CTA's last segment: nothing is loaded any more, so rows 64..127 take the packed ring as their
             // image instead of waiting for rows 0..63 to leave theirs
@@ -363,8 +374,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             uint8_t *srow_g = gbase + (srow - base);
             // 8-byte index in vis of (this row, tile column img0) -- formal when that column is left of the diagonal:
             // only its parity and offsets from it are used
-            const long long gi0 = (long long)(sg.f * cpt + cs) * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl +
-                                  (y0 + img0 - cs * sub - wo);
+            const long long gi0 = (long long)chan * Bn + (long long)xl * p.n_out - (long long)xl * (xl - 1) / 2 - xl + (y0 + img0 - coff);
             int2 *gimg = reinterpret_cast<int2 *>(p.vis) + gi0;
             const uint32_t par = (uint32_t)(reinterpret_cast<uintptr_t>(gimg) >> 3) & 1u;
             ptx::bulk_wait_read0();  // this thread's previous row segment has left shared memory
@@ -380,13 +390,13 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             int jlo, jhi;
             if (diag) {
                 jlo = max(64 * h, r);
-                jhi = min(64 * h + 64, cs * sub + p.n_out - x0 + wo);
+                jhi = min(64 * h + 64, coff + p.n_out - x0);
                 if (sub == 64 && h != cs) jhi = jlo;
             } else {
                 jlo = 64 * h;
                 jhi = min(64 * h + 64, p.n_out - y0);
             }
-            const bool row_ok = xl >= 0 && xl < p.n_out && (sub != 64 || sg.f * cpt + cs < p.f_out);
+            const bool row_ok = win_valid && xl >= 0 && xl < p.n_out && (sub != 64 || chan < p.f_out);
             if (GENERAL && !last && q >= 2) ptx::named_bar_sync(2, 32 * TD_EPI_WARPS);   // rows 0..63 have left the image
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -394,7 +404,7 @@ corr_tcd_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 // warp-uniform: the chunk is left of the diagonal for every row of the warp, outside the matrix, or
                 // (two channels per tile) in the other channel's columns
                 bool skip;
-                if (diag) skip = (col + 15 < 32 * q) || (sub == 128 ? (x0 + col >= p.n_out + wo || x0 + 32 * q >= p.n_out + wo) : ((col >> 6) != (q >> 1)));
+                if (diag) skip = (col + 15 < 32 * q) || (sub == 128 ? (x0 + col >= cend || x0 + 32 * q >= cend) : ((col >> 6) != (q >> 1)));
                 else skip = (y0 + col >= p.n_out) || (x0 + 32 * q >= p.n_out);
                 if (!skip) {
                     uint32_t ir[16], rr[16], ri[16];

@@ -227,12 +227,15 @@ def test_diagonal_block_kernel(corr, oracle, shape, shares, monkeypatch):
 
 
 @pytest.mark.parametrize("shape", [(100, 64, 3000), (100, 4, 777), (113, 16, 1000), (65, 16, 20000), (72, 2, 300), (97, 32, 257),
-                                   (104, 6, 5000)])
+                                   (104, 6, 5000), (37, 16, 3000), (37, 128, 700), (50, 8, 20000), (20, 12, 1000), (10, 8, 300),
+                                   (5, 16, 257), (3, 32, 1000), (1, 16, 100), (56, 6, 900), (24, 10, 4000)])
 def test_unpadded_stream_through_aligned_windows(corr, oracle, shape, monkeypatch):
     # N % 16 != 0, N <= 113 and rows of a multiple of 16 bytes: corr_tcd_kernel reads the stream as it is, channel f through
     # the 128-byte window at column f N rounded down to 16 (its inputs are rows / columns (f N) % 16 ... of the tile; what the
-    # window holds of the neighbouring channels is computed and dropped).  Both schedules; a buffer that is not 16-byte
-    # aligned takes the padded copy instead; same bits either way
+    # window holds of the neighbouring channels is computed and dropped).  N <= 56: several whole channels per window, tile g
+    # holds channels g c ... g c + c - 1, c = 113 // N (and AUTO takes this route instead of a padded copy + the warp-MMA
+    # kernel).  Both schedules; a buffer that is not 16-byte aligned takes the padded copy instead (same bits), or is
+    # refused when a window holds several channels
     import torch
     N, F, T = shape
     packed = workloads.uniform_bytes(N, F, T, seed=N + F + T)
@@ -240,13 +243,17 @@ def test_unpadded_stream_through_aligned_windows(corr, oracle, shape, monkeypatc
     for shares in ("0", "1"):
         monkeypatch.setenv("CORR_TCD_SHARES", shares)
         for off in (0, 3):
-            with corr.Plan(N, F, T, corr.PATH_TCGEN05) as plan:
-                assert plan.info["kernels"] == 1
+            with corr.Plan(N, F, T, corr.PATH_AUTO if N < 64 else corr.PATH_TCGEN05) as plan:
+                assert plan.info["kernels"] == 1 and plan.info["path"] == corr.PATH_TCGEN05
                 raw = torch.full((packed.size + 64,), 0x88, dtype=torch.uint8, device="cuda")
                 dev = raw[off:off + packed.size].view(T, F, N)
                 dev.copy_(torch.from_numpy(packed))
                 vis = plan.new_vis()
                 vis.fill_(-559038737)
+                if off and N <= 56:
+                    with pytest.raises(corr.CorrError, match="16-byte aligned"):
+                        plan.execute(dev, vis)
+                    continue
                 plan.execute(dev, vis)
                 torch.cuda.synchronize()
                 assert np.array_equal(vis.cpu().numpy(), want), (shape, shares, off)
@@ -433,6 +440,23 @@ def test_int32_headroom_edge(corr):
     got, info = _run(corr, packed, corr.PATH_TCGEN05)
     assert info["slices"] > 1
     assert (got[..., 0] == 128 * T).all() and (got[..., 1] == 0).all()
+
+
+def test_imma_ring_barriers_under_repetition(corr):
+    # regression: with one barrier per ring position (six positions, four K-split groups) a group waited for the same
+    # parity on every visit and, when TMA loads completed out of order, took another group's phase for its own: launch
+    # failures in about half of such loops, at this size, after the pad copy.  300 calls, then the same bits as the
+    # tcgen05 path
+    import torch
+    N, F, T = 24, 128, 65536
+    dev = torch.randint(0, 256, (T, F, N), dtype=torch.uint8, device="cuda")
+    with corr.Plan(N, F, T, corr.PATH_IMMA) as plan, corr.Plan(N, F, T, corr.PATH_TCGEN05) as ref:
+        vis = plan.new_vis()
+        for _ in range(300):
+            plan.execute(dev, vis)
+        want = ref.execute(dev)
+        torch.cuda.synchronize()
+        assert torch.equal(vis, want)
 
 
 @pytest.mark.parametrize("N,F", [(16, 2368), (32, 592), (48, 296), (64, 296)])
