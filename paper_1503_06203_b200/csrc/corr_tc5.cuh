@@ -158,15 +158,21 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
     const uint32_t bar0 = sum0 + T5_SUMS_BYTES;
     uint8_t *epi_g = gbase + (epi0 - base);
     int2 *sums_g = reinterpret_cast<int2 *>(gbase + (sum0 - base));   // [2][256] (K, R)
-    auto pk_full = [&](int s) { return bar0 + 8u * s; };
-    auto pk_empty = [&](int s) { return bar0 + 8u * (T5_PK + s); };
-    auto pl_full = [&](int s) { return bar0 + 8u * (2 * T5_PK + s); };
-    auto pl_empty = [&](int s) { return bar0 + 8u * (2 * T5_PK + T5_SLOTS + s); };
-    const uint32_t acc_full = bar0 + 8u * (2 * T5_PK + 2 * T5_SLOTS);
+    // packed ring: one pair of barriers per (position, parity of the stage).  The stages go alternately to the unpack groups
+    // {0, 1} and {2, 3}; with an odd number of positions a pair of groups comes back to a position only every second time
+    // round and, on a barrier per position, would always wait for the same parity: when TMA loads complete out of order
+    // it could take the other pair's not-yet-landed stage for its own (the hazard found in corr_imma_kernel,
+    // profiles/r02_secondary_kernels.md).  A (position, parity) pair is used once every T5_PK_PERIOD stages.
+    constexpr int T5_PK_PERIOD = (T5_PK % 2 == 0) ? T5_PK : 2 * T5_PK;
+    auto pk_full = [&](int s, int par) { return bar0 + 8u * (2 * s + par); };
+    auto pk_empty = [&](int s, int par) { return bar0 + 8u * (2 * T5_PK + 2 * s + par); };
+    auto pl_full = [&](int s) { return bar0 + 8u * (4 * T5_PK + s); };
+    auto pl_empty = [&](int s) { return bar0 + 8u * (4 * T5_PK + T5_SLOTS + s); };
+    const uint32_t acc_full = bar0 + 8u * (4 * T5_PK + 2 * T5_SLOTS);
     const uint32_t acc_empty = acc_full + 8u;
     auto sums_full = [&](int b) { return acc_empty + 8u + 8u * b; };
     const uint32_t tmem_slot = acc_empty + 24u;
-    static_assert(8 * (2 * T5_PK + 2 * T5_SLOTS) + 48 <= 512, "barrier area");
+    static_assert(8 * (4 * T5_PK + 2 * T5_SLOTS) + 48 <= 512, "barrier area");
     volatile uint32_t *tmem_slot_g = reinterpret_cast<volatile uint32_t *>(gbase + (tmem_slot - base));
     volatile int *claim_g = reinterpret_cast<volatile int *>(gbase + (tmem_slot + 8u - base));
 
@@ -178,8 +184,10 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         ptx::prefetch_tmap(&tmap_x);
         ptx::prefetch_tmap(&tmap_y);
         for (int s = 0; s < T5_PK; ++s) {
-            ptx::mbar_init(pk_full(s), 1);
-            ptx::mbar_init(pk_empty(s), 8);       // the two warp groups that own the two halves of the stage
+            for (int par = 0; par < 2; ++par) {
+                ptx::mbar_init(pk_full(s, par), 1);
+                ptx::mbar_init(pk_empty(s, par), 8);   // the two warp groups that own the two halves of the stage
+            }
         }
         for (int s = 0; s < T5_SLOTS; ++s) {
             ptx::mbar_init(pl_full(s), 8);        // one warp group of BOTH CTAs; the leader's copy is used
@@ -209,7 +217,7 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         // ===================== S1: TMA producer (each CTA loads its own blocks) =====================
         if (lane == 0) {
             int st = 0;
-            uint32_t ph = 0;
+            uint32_t pj = 0;   // stages loaded so far: stage pj goes to position pj % T5_PK and to the groups of parity pj & 1
             while (tc3_next_segment(p, sit, sg)) {
                 const int f = sg.f;
                 const ushort4 tile = sg.tile;
@@ -218,12 +226,17 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                 const int yc = tile.z * 128 + (int)rank * 64;
                 const int t_pad = t_begin + sg.cnt * T3_GROUP;
                 for (int t = t_begin; t < t_pad; t += T5_ST) {
-                    ptx::mbar_wait(pk_empty(st), ph ^ 1u);
+                    if (pj >= (uint32_t)T5_PK) {   // the position's last stage, pj - T5_PK, has been read by its groups
+                        const uint32_t jp = pj - T5_PK;
+                        ptx::mbar_wait(pk_empty(st, (int)(jp & 1u)), (jp / T5_PK_PERIOD) & 1u);
+                    }
                     const uint32_t dst = pk0 + st * T5_PK_BYTES;
-                    ptx::mbar_arrive_expect_tx(pk_full(st), T5_PK_BYTES);
-                    ptx::tma_load_3d(dst, &tmap_x, pk_full(st), xc, f, t);
-                    ptx::tma_load_3d(dst + T5_XBYTES, &tmap_y, pk_full(st), yc, f, t);
-                    if (++st == T5_PK) { st = 0; ph ^= 1u; }
+                    const int par = (int)(pj & 1u);
+                    ptx::mbar_arrive_expect_tx(pk_full(st, par), T5_PK_BYTES);
+                    ptx::tma_load_3d(dst, &tmap_x, pk_full(st, par), xc, f, t);
+                    ptx::tma_load_3d(dst + T5_XBYTES, &tmap_y, pk_full(st, par), yc, f, t);
+                    ++pj;
+                    if (++st == T5_PK) st = 0;
                 }
             }
         }
@@ -290,7 +303,11 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
         const int tb = 4 * (lane & 3);          // first sample of r0 / r1 inside the slot (r2 / r3: + 16)
         // ring positions of this group's next slot o = grp, grp + 4, ... (segments hold multiples of 8 slots)
         int st = (grp >> 1) % T5_PK;
-        uint32_t sph = 0, pph = 0;
+        const int spar = grp >> 1;              // parity of the stages this group reads
+        const int st0 = st;                     // the walk st, st + 2, ... (mod T5_PK) is back here after T5_PK_PERIOD stages:
+        uint32_t sph = 0, pph = 0;              // that is when the phase of this group's (position, parity) barriers flips
+        const uint32_t pkb = bar0 + 8u * (uint32_t)spar;   // pk_full(s, spar) = pkb + 16 s,  pk_empty(s, spar) = pkb + 16 (T5_PK + s)
+        static_assert(T5_PK % 2 == 1, "an even ring: the walk returns after T5_PK / 2 steps and st0 marks that as well");
         int seg_no = 0;
         while (tc3_next_segment(p, sit, sg)) {
             const int nslots = sg.cnt * (T3_GROUP / T5_KS);
@@ -298,7 +315,7 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
             uint32_t sxw[4] = {0, 0, 0, 0}, sxl[4] = {0, 0, 0, 0};   // x inputs 32 q + lane / 4 + 8 j
             uint32_t syw[2] = {0, 0}, syl[2] = {0, 0};            // y inputs 16 q + lane / 4 + 8 j of this CTA's half
             for (int j = grp; j < nslots; j += T5_GROUPS, valid -= T5_KS * T5_GROUPS) {
-                ptx::mbar_wait(pk_full(st), pph);
+                ptx::mbar_wait(pkb + 16u * (uint32_t)st, pph);
                 uint32_t xa[4], xb[4], ya[4];
                 const uint32_t xsrc = xinv + (uint32_t)st * T5_PK_BYTES;
                 ptx::ldsm_t_b8_x2(xsrc, xa[0], xa[1], xa[2], xa[3]);         // inputs 32q + 0..15
@@ -319,7 +336,7 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
 #pragma unroll
                 for (int k = 0; k < 4; ++k) { al[k] = xa[k] & 0x0F0F0F0Fu; al[4 + k] = xb[k] & 0x0F0F0F0Fu; yl[k] = ya[k] & 0x0F0F0F0Fu; }
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(pk_empty(st));   // every byte this warp needs is in registers
+                if (lane == 0) ptx::mbar_arrive(pkb + 16u * (uint32_t)(T5_PK + st));   // every byte this warp needs is in registers
                 ptx::mbar_wait_cluster(my_empty, sph ^ 1u);
                 ptx::tmem_st_16x128b_x2(ta, xa[0], xa[1], xa[2], xa[3]);
                 ptx::tmem_st_16x128b_x2(ta + (16u << 16), xb[0], xb[1], xb[2], xb[3]);
@@ -362,7 +379,8 @@ corr_tc5_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constan
                 if (lane == 0) ptx::mbar_arrive_cluster(my_full, 0);  // the leader's barrier
                 // next slot of this group: o += 4 (two stages on, the same ring entry)
                 sph ^= 1u;
-                st += 2; if (st >= T5_PK) { st -= T5_PK; pph ^= 1u; }
+                st += 2; if (st >= T5_PK) st -= T5_PK;
+                if (st == st0) pph ^= 1u;
             }
             // ---- the sums of this segment: reduce over the four lanes that share an input, then into the segment's
             //      buffer (x rows: own CTA; y columns: both CTAs of the pair)
